@@ -1,0 +1,180 @@
+/* cbct.h -- C ABI of the B200-native (sm_100a) hot path of tight-frame-regularised cone-beam CT
+ * reconstruction (arxiv/paper_1008_2042: Jia, Dong, Lou, Jiang).
+ *
+ * Citations are "/root/reference/PAPER.md:<line> (section / equation)" plus the reading of
+ * SURVEY.md §8(c) where the paper is silent.  All kernels are hand-written CUDA for sm_100a;
+ * there is NO CPU fallback and no other backend: on a device that is not compute capability 10.x
+ * every entry point that would launch a kernel returns CBCT_E_UNSUPPORTED.
+ *
+ * Conventions (all entry points)
+ *   - Lengths in mm, angles in rad.  Volumes are f[z][y][x] (x fastest), projections g[view][v][u]
+ *     (u fastest), tight-frame coefficients alpha[27][z][y][x] with band i = l + 3m + 9n (l on x).
+ *     Everything is contiguous fp32.
+ *   - Pointers named d_* are DEVICE pointers, 16-byte aligned, owned by the caller (e.g. a PyTorch
+ *     tensor's data_ptr()).  Pointers named h_* are HOST pointers.  `stream` is a cudaStream_t passed
+ *     as void* (NULL = the legacy default stream).
+ *   - in and out must not alias unless a function says "in place".  Outputs are overwritten.
+ *   - Hot calls are asynchronous on `stream`, allocate nothing and never synchronise the host; they
+ *     return launch errors only.  Handles own their device workspace (allocated at *_create).
+ *   - Return value: 0 = CBCT_OK, < 0 = error, CBCT_BREAKDOWN (+1) = CGLS breakdown (not a failure).
+ *     Nothing throws or aborts.
+ */
+#ifndef CBCT_H
+#define CBCT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    CBCT_OK = 0,
+    CBCT_E_INVALID = -1,      /* bad argument (null pointer, non-positive size, geometry rejected) */
+    CBCT_E_UNSUPPORTED = -2,  /* no sm_100-class device / feature not available */
+    CBCT_E_CUDA = -3,         /* a CUDA runtime call failed; see cbct_last_cuda_error() */
+    CBCT_BREAKDOWN = 1        /* CGLS: gamma == 0 or ||q||^2 == 0 (PAPER.md:446, :461 would divide by 0) */
+};
+
+/* Static string for a status code. */
+const char *cbct_status_string(int status);
+/* Raw cudaError_t of the last CBCT_E_CUDA seen on the calling thread (0 if none). */
+int cbct_last_cuda_error(void);
+/* Library version, e.g. 100 = 1.0.0. */
+int cbct_version(void);
+
+/* ------------------------------------------------------------------------------------------------
+ * Geometry: circular orbit, flat panel (Eq. 1, Fig. 1 caption).
+ * Frame (the figure itself is missing from the paper text): origin = isocentre,
+ * z = rotation axis, source x_S = (SAD cos th, SAD sin th, 0), detector centre
+ * c_D = -(SDD-SAD)(cos th, sin th, 0), e_u = (-sin th, cos th, 0), e_v = (0,0,1).
+ * Voxel centre x = ox + (ix-(nx-1)/2) dx; pixel centre u = u0 + (iu-(nu-1)/2) du.  One ray per pixel
+ * centre.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t nx, ny, nz;       /* volume size in voxels */
+    double dx, dy, dz;        /* voxel pitch */
+    double ox, oy, oz;        /* volume centre offset from the isocentre */
+    int32_t nu, nv;           /* detector size in pixels */
+    double du, dv;            /* pixel pitch */
+    double u0, v0;            /* detector centre offset */
+    double sad, sdd;          /* source-axis and source-detector distance */
+    int32_t n_views;
+    const double *angles;     /* HOST array[n_views]; copied at create */
+    double step_mm;           /* sampling step; <= 0 selects 0.5*min(dx,dy,dz) */
+} cbct_geometry_desc;
+
+typedef struct cbct_geometry cbct_geometry; /* opaque; owns device-side per-view tables + workspace */
+
+/* Validates and builds a geometry handle on the current CUDA device.
+ * CBCT_E_INVALID: null pointers, non-positive sizes/pitches, sad <= 0, sdd <= sad, or the padded
+ * volume's bounding radius R >= SAD (source inside the volume).  Synchronous; allocates. */
+int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometry **out);
+int cbct_geometry_destroy(cbct_geometry *geom);
+
+/* Derived quantities (any out pointer may be NULL):
+ *   n_vox, n_rays; K, t_min, step_mm of the global sample grid t_k = t_min + (k+1/2) step,
+ *   t_min = SAD - R, K = ceil(2R/step), R = half-diagonal of the zero-padded box;
+ *   n_samples_algorithmic = sum over rays of chord(padded box)/step (the unit of "Gsamples/s");
+ *   workspace_bytes = device memory owned by the handle. */
+int cbct_geometry_info(const cbct_geometry *geom, int64_t *n_vox, int64_t *n_rays, int32_t *K,
+                       double *t_min, double *step_mm, int64_t *n_samples_algorithmic,
+                       size_t *workspace_bytes);
+
+/* g = P f.  PAPER.md:73 Eq. 1 discretised as step * sum_k T[f](x_S + n t_k), T = zero-padded
+ * trilinear interpolation (north_star).  d_vol: nx*ny*nz, d_proj: n_views*nv*nu. */
+int cbct_forward(const cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
+
+/* f = P^T g, the exact matrix transpose of cbct_forward ("f = P^T g"; north_star),
+ * voxel-driven and deterministic (no atomics).  d_proj: n_views*nv*nu, d_vol: nx*ny*nz. */
+int cbct_backproject(const cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
+
+/* Host-buffer variants (used for end-to-end timing): copy h_in -> device workspace, run, copy the
+ * result to h_out, all on `stream`; the caller synchronises the stream.  Pinned host memory makes
+ * the copies asynchronous. */
+int cbct_forward_host(cbct_geometry *geom, const float *h_vol, float *h_proj, void *stream);
+int cbct_backproject_host(cbct_geometry *geom, const float *h_proj, float *h_vol, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * CGLS (Appendix 1).  State vectors x, p (volume size) and r (projection size) are
+ * the caller's; the handle owns q (projection size), s (volume size) and the fp64 device scalars.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct cbct_cgls cbct_cgls;
+int cbct_cgls_create(const cbct_geometry *geom, cbct_cgls **out);
+int cbct_cgls_destroy(cbct_cgls *cg);
+
+/* Initialize: r = g - P x0; p = s = P^T r; gamma = ||s||^2.  d_x holds x0. */
+int cbct_cgls_init(cbct_cgls *cg, const float *d_g, const float *d_x, float *d_r, float *d_p, void *stream);
+
+/* One pass through steps 1-7: q = P p; alpha = gamma/||q||^2; x += alpha p;
+ * r -= alpha q; s = P^T r; gamma' = ||s||^2; beta = gamma'/gamma; p = s + beta p.
+ * All scalars stay on the device (fp64).  On breakdown (gamma == 0 or ||q||^2 == 0) the step leaves
+ * x, r, p unchanged and sets the device flag; still returns CBCT_OK because
+ * the host is never synchronised here -- read the flag with cbct_cgls_scalars. */
+int cbct_cgls_step(cbct_cgls *cg, float *d_x, float *d_r, float *d_p, void *stream);
+
+/* Synchronises `stream` and copies out {gamma, ||q||^2, alpha, beta, ||r||^2}.  ||r||^2 is computed
+ * here from d_r if d_r != NULL, else reported as -1.  Returns CBCT_BREAKDOWN if the flag is set. */
+int cbct_cgls_scalars(cbct_cgls *cg, const float *d_r, double out[5], void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Piecewise-linear tight frame: h0 = 1/4[1,2,1], h1 = sqrt(2)/4[1,0,-1],
+ * h2 = 1/4[-1,2,-1]; psi_i = h_l(x) h_m(y) h_n(z); alpha_i = psi_i (*) f (true convolution),
+ * edge-replicate extension of f; D^T is the exact transpose.
+ * ---------------------------------------------------------------------------------------------- */
+int tf_decompose(const float *d_f, float *d_alpha, int nx, int ny, int nz, void *stream);
+/* Vector shrinkage T_mu, Eq. 2, in place on bands 1..26 (band 0 untouched);
+ * factor max(1 - mu/||alpha_h||, 0), := 0 where ||alpha_h|| = 0. */
+int tf_shrink(float *d_alpha, float mu, int nx, int ny, int nz, void *stream);
+/* f = D^T alpha = sum_i psi_i(-x) (*) alpha_i. */
+int tf_reconstruct(const float *d_alpha, float *d_f, int nx, int ny, int nz, void *stream);
+/* f_out = [H] D^T T_mu D f_in without materialising alpha (H = max(.,0), PAPER.md:131,
+ * applied when clamp_nonneg != 0).  d_in != d_out. */
+int tf_apply_fused(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz,
+                   void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Multigrid transfers (§2.2.3).  Per-axis factors fx,fy,fz in {1,2}; fine sizes must be
+ * divisible.  restrict = mean of the children; prolong = cell-centred linear interpolation (weights
+ * 3/4, 1/4, neighbour clamped at the faces).
+ * ---------------------------------------------------------------------------------------------- */
+int mg_restrict(const float *d_fine, float *d_coarse, int nx_f, int ny_f, int nz_f, int fx, int fy, int fz,
+                void *stream);
+int mg_prolong(const float *d_coarse, float *d_fine, int nx_f, int ny_f, int nz_f, int fx, int fy, int fz,
+               void *stream);
+
+/* Algorithm A2 step 1 (garbled; reading of SURVEY.md §8(c) item 11):
+ * v = f_cur + coef (f_cur - f_prev), coef = (t^(k-1) - 1)/t^(k).  n = element count. */
+int cbct_a2_extrapolate(const float *d_f_cur, const float *d_f_prev, float *d_v, float coef, int64_t n,
+                        void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Driver: Algorithm A2 inside the coarse-to-fine multigrid cascade
+ * (PAPER.md:232): levels coarsen x,y by 2 each, z kept, g at full resolution; n_outer[] is
+ * coarse -> fine (PAPER.md:288 uses 5/10/15); n_cgls passes of CGLS steps 1-7 per outer iteration
+ * ("M = 2~3"); one mu for all levels; momentum = 0 gives Algorithm A1.
+ * d_f receives the finest-level volume.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct cbct_recon cbct_recon; /* opaque; owns per-level geometry, CGLS state and volumes */
+/* Allocates everything the cascade needs (finest nx, ny must be divisible by 2^(n_levels-1)). */
+int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels, cbct_recon **out);
+int cbct_recon_destroy(cbct_recon *recon);
+/* Runs the cascade asynchronously on `stream` (no allocation, no host synchronisation). */
+int cbct_recon_run(cbct_recon *recon, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu,
+                   int momentum, void *stream);
+/* HOST buffers: h_g -> device, run, volume -> h_f; synchronises `stream` before returning. */
+int cbct_recon_run_host(cbct_recon *recon, const float *h_g, float *h_f, const int *n_outer, int n_cgls,
+                        float mu, int momentum, void *stream);
+
+/* One-shot convenience wrappers: create + run + synchronise + destroy. */
+int cbct_tf_reconstruct(const cbct_geometry_desc *finest, const float *d_g, float *d_f, int n_levels,
+                        const int *n_outer, int n_cgls, float mu, int momentum, void *stream);
+/* Same with HOST buffers: copies h_g to the device, reconstructs, copies the volume back to h_f. */
+int cbct_tf_reconstruct_host(const cbct_geometry_desc *finest, const float *h_g, float *h_f, int n_levels,
+                             const int *n_outer, int n_cgls, float mu, int momentum, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBCT_H */

@@ -1,0 +1,321 @@
+"""Thin ctypes binding of libcbct_b200.so (include/cbct.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing, or a call returns
+an error status, this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcbct_b200.so")
+
+CBCT_OK, CBCT_E_INVALID, CBCT_E_UNSUPPORTED, CBCT_E_CUDA, CBCT_BREAKDOWN = 0, -1, -2, -3, 1
+
+# every symbol include/cbct.h declares (tests check the library exports all of them)
+EXPORTS = [
+    "cbct_status_string", "cbct_last_cuda_error", "cbct_version",
+    "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
+    "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
+    "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
+    "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
+    "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
+    "cbct_recon_create", "cbct_recon_destroy", "cbct_recon_run", "cbct_recon_run_host",
+    "cbct_tf_reconstruct", "cbct_tf_reconstruct_host",
+]
+
+
+class CbctError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().cbct_status_string(status).decode()
+        extra = f" (cudaError {lib().cbct_last_cuda_error()})" if status == CBCT_E_CUDA else ""
+        super().__init__(f"{where}: {msg}{extra}")
+
+
+class GeometryDesc(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("ox", C.c_double), ("oy", C.c_double), ("oz", C.c_double),
+                ("nu", C.c_int32), ("nv", C.c_int32),
+                ("du", C.c_double), ("dv", C.c_double), ("u0", C.c_double), ("v0", C.c_double),
+                ("sad", C.c_double), ("sdd", C.c_double),
+                ("n_views", C.c_int32), ("angles", C.POINTER(C.c_double)),
+                ("step_mm", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library (once).  Fails loudly when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1008_2042_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, fp, ip = C.c_void_p, C.c_void_p, C.c_int
+    L.cbct_status_string.restype = C.c_char_p
+    L.cbct_status_string.argtypes = [ip]
+    L.cbct_last_cuda_error.argtypes = []
+    L.cbct_version.argtypes = []
+    L.cbct_geometry_create.argtypes = [C.POINTER(GeometryDesc), C.POINTER(vp)]
+    L.cbct_geometry_destroy.argtypes = [vp]
+    L.cbct_geometry_info.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32),
+                                     C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64),
+                                     C.POINTER(C.c_size_t)]
+    for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host"):
+        getattr(L, name).argtypes = [vp, fp, fp, vp]
+    L.cbct_cgls_create.argtypes = [vp, C.POINTER(vp)]
+    L.cbct_cgls_destroy.argtypes = [vp]
+    L.cbct_cgls_init.argtypes = [vp, fp, fp, fp, fp, vp]
+    L.cbct_cgls_step.argtypes = [vp, fp, fp, fp, vp]
+    L.cbct_cgls_scalars.argtypes = [vp, fp, C.POINTER(C.c_double), vp]
+    L.tf_decompose.argtypes = [fp, fp, ip, ip, ip, vp]
+    L.tf_shrink.argtypes = [fp, C.c_float, ip, ip, ip, vp]
+    L.tf_reconstruct.argtypes = [fp, fp, ip, ip, ip, vp]
+    L.tf_apply_fused.argtypes = [fp, fp, C.c_float, ip, ip, ip, ip, vp]
+    L.mg_restrict.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
+    L.mg_prolong.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
+    L.cbct_a2_extrapolate.argtypes = [fp, fp, fp, C.c_float, C.c_int64, vp]
+    L.cbct_recon_create.argtypes = [C.POINTER(GeometryDesc), ip, C.POINTER(vp)]
+    L.cbct_recon_destroy.argtypes = [vp]
+    L.cbct_recon_run.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
+    L.cbct_recon_run_host.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
+    L.cbct_tf_reconstruct.argtypes = [C.POINTER(GeometryDesc), fp, fp, ip, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
+    L.cbct_tf_reconstruct_host.argtypes = [C.POINTER(GeometryDesc), fp, fp, ip, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
+    for name in EXPORTS:
+        if name != "cbct_status_string":
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(status: int, where: str, allow_breakdown: bool = False) -> int:
+    if status == CBCT_OK or (allow_breakdown and status == CBCT_BREAKDOWN):
+        return status
+    raise CbctError(status, where)
+
+
+def _stream(stream=None) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dptr(t, n: Optional[int] = None) -> int:
+    """Device pointer of a contiguous fp32 CUDA tensor (marshalling only)."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float32 CUDA tensor")
+    if n is not None and t.numel() != n:
+        raise ValueError(f"expected {n} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+def _hptr(t, n: Optional[int] = None) -> int:
+    """Host pointer of a contiguous fp32 CPU tensor / numpy array."""
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float32 or not t.flags.c_contiguous:
+            raise TypeError("expected a C-contiguous float32 array")
+        if n is not None and t.size != n:
+            raise ValueError(f"expected {n} elements, got {t.size}")
+        return t.ctypes.data
+    import torch
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float32 CPU tensor")
+    if n is not None and t.numel() != n:
+        raise ValueError(f"expected {n} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+def make_desc(geom):
+    """GeometryDesc (+ the angle array that must outlive it) from any object with the fields of
+    synthetic.Geometry."""
+    ang = np.ascontiguousarray(np.asarray(list(geom.angles), dtype=np.float64))
+    d = GeometryDesc(geom.nx, geom.ny, geom.nz, geom.dx, geom.dy, geom.dz, geom.ox, geom.oy, geom.oz,
+                     geom.nu, geom.nv, geom.du, geom.dv, geom.u0, geom.v0, geom.sad, geom.sdd,
+                     len(ang), ang.ctypes.data_as(C.POINTER(C.c_double)), float(getattr(geom, "step_mm", 0.0)))
+    return d, ang
+
+
+class Geometry:
+    """cbct_geometry handle."""
+
+    def __init__(self, geom):
+        self.spec = geom
+        d, keep = make_desc(geom)
+        h = C.c_void_p()
+        _check(lib().cbct_geometry_create(C.byref(d), C.byref(h)), "cbct_geometry_create")
+        self.handle = h
+        nv, nr, K = C.c_int64(), C.c_int64(), C.c_int32()
+        t0, st, ns, ws = C.c_double(), C.c_double(), C.c_int64(), C.c_size_t()
+        _check(lib().cbct_geometry_info(h, C.byref(nv), C.byref(nr), C.byref(K), C.byref(t0), C.byref(st),
+                                        C.byref(ns), C.byref(ws)), "cbct_geometry_info")
+        self.n_vox, self.n_rays, self.K = nv.value, nr.value, K.value
+        self.t_min, self.step_mm, self.n_samples, self.workspace_bytes = t0.value, st.value, ns.value, ws.value
+        self.vol_shape = (geom.nz, geom.ny, geom.nx)
+        self.proj_shape = (len(tuple(geom.angles)), geom.nv, geom.nu)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().cbct_geometry_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def forward(self, d_vol, d_proj, stream=None):
+        _check(lib().cbct_forward(self.handle, _dptr(d_vol, self.n_vox), _dptr(d_proj, self.n_rays), _stream(stream)),
+               "cbct_forward")
+        return d_proj
+
+    def backproject(self, d_proj, d_vol, stream=None):
+        _check(lib().cbct_backproject(self.handle, _dptr(d_proj, self.n_rays), _dptr(d_vol, self.n_vox),
+                                      _stream(stream)), "cbct_backproject")
+        return d_vol
+
+    def forward_host(self, h_vol, h_proj, stream=None):
+        _check(lib().cbct_forward_host(self.handle, _hptr(h_vol, self.n_vox), _hptr(h_proj, self.n_rays),
+                                       _stream(stream)), "cbct_forward_host")
+        return h_proj
+
+    def backproject_host(self, h_proj, h_vol, stream=None):
+        _check(lib().cbct_backproject_host(self.handle, _hptr(h_proj, self.n_rays), _hptr(h_vol, self.n_vox),
+                                           _stream(stream)), "cbct_backproject_host")
+        return h_vol
+
+
+class Cgls:
+    """cbct_cgls handle."""
+
+    def __init__(self, geometry: Geometry):
+        self.geometry = geometry
+        h = C.c_void_p()
+        _check(lib().cbct_cgls_create(geometry.handle, C.byref(h)), "cbct_cgls_create")
+        self.handle = h
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().cbct_cgls_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def init(self, d_g, d_x, d_r, d_p, stream=None):
+        G = self.geometry
+        _check(lib().cbct_cgls_init(self.handle, _dptr(d_g, G.n_rays), _dptr(d_x, G.n_vox), _dptr(d_r, G.n_rays),
+                                    _dptr(d_p, G.n_vox), _stream(stream)), "cbct_cgls_init")
+
+    def step(self, d_x, d_r, d_p, stream=None):
+        G = self.geometry
+        _check(lib().cbct_cgls_step(self.handle, _dptr(d_x, G.n_vox), _dptr(d_r, G.n_rays), _dptr(d_p, G.n_vox),
+                                    _stream(stream)), "cbct_cgls_step")
+
+    def scalars(self, d_r=None, stream=None):
+        """dict(gamma, qq, alpha, beta, rr, breakdown); synchronises the stream."""
+        out = (C.c_double * 5)()
+        s = _check(lib().cbct_cgls_scalars(self.handle, _dptr(d_r, self.geometry.n_rays) if d_r is not None else None,
+                                           out, _stream(stream)), "cbct_cgls_scalars", allow_breakdown=True)
+        return dict(gamma=out[0], qq=out[1], alpha=out[2], beta=out[3], rr=out[4], breakdown=(s == CBCT_BREAKDOWN))
+
+
+def _dims(shape):
+    nz, ny, nx = shape
+    return int(nx), int(ny), int(nz)
+
+
+def tf_decompose(d_f, d_alpha, stream=None):
+    nx, ny, nz = _dims(d_f.shape)
+    _check(lib().tf_decompose(_dptr(d_f), _dptr(d_alpha, 27 * nx * ny * nz), nx, ny, nz, _stream(stream)), "tf_decompose")
+    return d_alpha
+
+
+def tf_shrink(d_alpha, mu: float, stream=None):
+    nx, ny, nz = _dims(d_alpha.shape[1:])
+    _check(lib().tf_shrink(_dptr(d_alpha, 27 * nx * ny * nz), float(mu), nx, ny, nz, _stream(stream)), "tf_shrink")
+    return d_alpha
+
+
+def tf_reconstruct(d_alpha, d_f, stream=None):
+    nx, ny, nz = _dims(d_f.shape)
+    _check(lib().tf_reconstruct(_dptr(d_alpha, 27 * nx * ny * nz), _dptr(d_f), nx, ny, nz, _stream(stream)),
+           "tf_reconstruct")
+    return d_f
+
+
+def tf_apply_fused(d_in, d_out, mu: float, clamp_nonneg: bool = False, stream=None):
+    nx, ny, nz = _dims(d_in.shape)
+    _check(lib().tf_apply_fused(_dptr(d_in), _dptr(d_out, nx * ny * nz), float(mu), int(bool(clamp_nonneg)), nx, ny, nz,
+                                _stream(stream)), "tf_apply_fused")
+    return d_out
+
+
+def mg_restrict(d_fine, d_coarse, fx=2, fy=2, fz=1, stream=None):
+    nx, ny, nz = _dims(d_fine.shape)
+    _check(lib().mg_restrict(_dptr(d_fine), _dptr(d_coarse, (nx // fx) * (ny // fy) * (nz // fz)), nx, ny, nz, fx, fy, fz,
+                             _stream(stream)), "mg_restrict")
+    return d_coarse
+
+
+def mg_prolong(d_coarse, d_fine, fx=2, fy=2, fz=1, stream=None):
+    nx, ny, nz = _dims(d_fine.shape)
+    _check(lib().mg_prolong(_dptr(d_coarse, (nx // fx) * (ny // fy) * (nz // fz)), _dptr(d_fine), nx, ny, nz, fx, fy, fz,
+                            _stream(stream)), "mg_prolong")
+    return d_fine
+
+
+def a2_extrapolate(d_f_cur, d_f_prev, d_v, coef: float, stream=None):
+    n = d_f_cur.numel()
+    _check(lib().cbct_a2_extrapolate(_dptr(d_f_cur), _dptr(d_f_prev, n), _dptr(d_v, n), float(coef), n, _stream(stream)),
+           "cbct_a2_extrapolate")
+    return d_v
+
+
+class Recon:
+    """cbct_recon handle: A2 inside the multigrid cascade."""
+
+    def __init__(self, geom, n_levels: int):
+        d, keep = make_desc(geom)
+        h = C.c_void_p()
+        _check(lib().cbct_recon_create(C.byref(d), int(n_levels), C.byref(h)), "cbct_recon_create")
+        self.handle, self.n_levels, self.spec = h, int(n_levels), geom
+        self.n_vox = geom.nx * geom.ny * geom.nz
+        self.n_rays = len(tuple(geom.angles)) * geom.nv * geom.nu
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().cbct_recon_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def _outer(self, n_outer: Sequence[int]):
+        assert len(n_outer) == self.n_levels
+        return (C.c_int * self.n_levels)(*[int(v) for v in n_outer])
+
+    def run(self, d_g, d_f, n_outer, n_cgls=3, mu=5e-4, momentum=True, stream=None):
+        _check(lib().cbct_recon_run(self.handle, _dptr(d_g, self.n_rays), _dptr(d_f, self.n_vox), self._outer(n_outer),
+                                    int(n_cgls), float(mu), int(bool(momentum)), _stream(stream)), "cbct_recon_run")
+        return d_f
+
+    def run_host(self, h_g, h_f, n_outer, n_cgls=3, mu=5e-4, momentum=True, stream=None):
+        _check(lib().cbct_recon_run_host(self.handle, _hptr(h_g, self.n_rays), _hptr(h_f, self.n_vox),
+                                         self._outer(n_outer), int(n_cgls), float(mu), int(bool(momentum)),
+                                         _stream(stream)), "cbct_recon_run_host")
+        return h_f
+
+
+def tf_reconstruct_volume(geom, d_g, d_f, n_levels, n_outer, n_cgls=3, mu=5e-4, momentum=True, stream=None):
+    """One-shot cbct_tf_reconstruct."""
+    d, keep = make_desc(geom)
+    arr = (C.c_int * n_levels)(*[int(v) for v in n_outer])
+    _check(lib().cbct_tf_reconstruct(C.byref(d), _dptr(d_g), _dptr(d_f), int(n_levels), arr, int(n_cgls), float(mu),
+                                     int(bool(momentum)), _stream(stream)), "cbct_tf_reconstruct")
+    return d_f

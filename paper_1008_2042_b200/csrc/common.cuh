@@ -1,0 +1,95 @@
+// common.cuh -- internal declarations shared by the CUDA translation units of libcbct_b200.
+// Nothing in this directory is shared with oracle/ (the fp64 checker) and vice versa.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+
+#include "../../include/cbct.h"
+
+namespace cbct {
+
+// ---- error plumbing -------------------------------------------------------------------------
+int set_cuda_error(cudaError_t e);          // records e for cbct_last_cuda_error(), returns CBCT_E_CUDA
+int device_supported();                     // CBCT_OK on a compute-capability-10.x device
+#define CBCT_CUDA_TRY(expr)                                        \
+    do {                                                           \
+        cudaError_t _e = (expr);                                   \
+        if (_e != cudaSuccess) return ::cbct::set_cuda_error(_e);  \
+    } while (0)
+#define CBCT_TRY(expr)                 \
+    do {                               \
+        int _s = (expr);               \
+        if (_s != CBCT_OK) return _s;  \
+    } while (0)
+#define CBCT_LAUNCH_CHECK() CBCT_CUDA_TRY(cudaGetLastError())
+
+static inline cudaStream_t as_stream(void *s) { return reinterpret_cast<cudaStream_t>(s); }
+static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// ---- device-side geometry (POD, passed by value to kernels) ------------------------------------
+// Index coordinates: X = x * inv_dx + cx  with cx = -ox/dx + (nx-1)/2.
+// Sample grid: tau_k = t_k - SAD = tau0 + k*step, tau0 = t_min + step/2 - SAD; rays are re-anchored at
+// t = SAD (near the isocentre) so that fp32 positions stay accurate.
+struct DevGeom {
+    int nx, ny, nz, nu, nv, n_views, K;
+    double sad, sdd, du, dv, u_first, v_first;   // u = u_first + iu*du
+    double inv_dx, inv_dy, inv_dz, cx, cy, cz;
+    double tau0, step;
+    const double2 *view_cs;                      // device: (cos th, sin th) per view
+};
+
+struct RayF {                                    // one ray in index space, fp32: P(tau) = c + b*tau
+    float cx, cy, cz, bx, by, bz;
+};
+
+// fp64 ray set-up, identical for P and P^T so both sample the same points.
+__device__ __forceinline__ void ray_setup(const DevGeom &g, int view, int iv, int iu, RayF &r,
+                                          double &bxd, double &byd, double &bzd, double &cxd, double &cyd,
+                                          double &czd) {
+    const double2 cs = g.view_cs[view];
+    const double u = g.u_first + iu * g.du, v = g.v_first + iv * g.dv;
+    const double ex = -g.sdd * cs.x - u * cs.y, ey = -g.sdd * cs.y + u * cs.x, ez = v;
+    const double invL = rsqrt(ex * ex + ey * ey + ez * ez);
+    const double nx_ = ex * invL, ny_ = ey * invL, nz_ = ez * invL;
+    // point at t = SAD
+    const double px = g.sad * cs.x + nx_ * g.sad, py = g.sad * cs.y + ny_ * g.sad, pz = nz_ * g.sad;
+    cxd = px * g.inv_dx + g.cx; cyd = py * g.inv_dy + g.cy; czd = pz * g.inv_dz + g.cz;
+    bxd = nx_ * g.inv_dx; byd = ny_ * g.inv_dy; bzd = nz_ * g.inv_dz;
+    r.cx = (float)cxd; r.cy = (float)cyd; r.cz = (float)czd;
+    r.bx = (float)bxd; r.by = (float)byd; r.bz = (float)bzd;
+}
+
+}  // namespace cbct
+
+// ---- opaque handles --------------------------------------------------------------------------------
+struct cbct_geometry {
+    cbct_geometry_desc desc;            // desc.angles points into `angles`
+    std::vector<double> angles;
+    double R, t_min, step;
+    int32_t K;
+    int64_t n_vox, n_rays, n_samples;
+    cbct::DevGeom dg;
+    double2 *d_view_cs;
+    float *d_ws_vol, *d_ws_proj;        // staging for the *_host entry points (allocated at create)
+    float *d_bp_partial;                // P^T workspace (per-corner partial volumes), may be null
+    size_t workspace_bytes;
+};
+
+struct cbct_cgls {
+    const cbct_geometry *geom;
+    float *d_q, *d_s;
+    double *d_scal;                     // {gamma, qq, alpha, beta, rr, gamma_new}
+    int *d_flag;                        // breakdown flag
+    double *d_partials;                 // reduction scratch
+    unsigned int *d_counter;
+};
+
+namespace cbct {
+// kernels' host launchers used across translation units
+int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
+int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
+int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,
+                 cudaStream_t st);
+constexpr int kReduceBlocks = 1184;     // 148 SMs x 8
+}  // namespace cbct

@@ -1,0 +1,146 @@
+// driver.cu -- Algorithm A2 inside the coarse-to-fine multigrid cascade
+// (PAPER.md:232): cbct_recon_* and the one-shot cbct_tf_reconstruct*.  The host only sequences
+// launches: the t-sequence of A2 step 5 is data independent, so nothing is read back and the whole
+// reconstruction is one asynchronous stream of kernels.
+#include <cmath>
+#include <new>
+
+#include "common.cuh"
+
+struct cbct_recon_level {
+    cbct_geometry *geom;
+    cbct_cgls *cg;
+    float *d_x, *d_p, *d_fa, *d_fb, *d_fc;   // volume-sized: CGLS x, p; A2 f^(k), f^(k-1), scratch
+    int nx, ny, nz;
+};
+
+struct cbct_recon {
+    int n_levels;
+    std::vector<cbct_recon_level> lev;       // coarse -> fine
+    float *d_r;                               // projection-sized CGLS residual (g is full size on every level)
+    float *d_g, *d_f;                         // staging for the host entry point
+    int64_t n_rays, n_vox_finest;
+};
+
+using namespace cbct;
+
+extern "C" int cbct_recon_destroy(cbct_recon *R) {
+    if (!R) return CBCT_OK;
+    for (auto &L : R->lev) {
+        cbct_cgls_destroy(L.cg);
+        cbct_geometry_destroy(L.geom);
+        cudaFree(L.d_x); cudaFree(L.d_p); cudaFree(L.d_fa); cudaFree(L.d_fb); cudaFree(L.d_fc);
+    }
+    cudaFree(R->d_r); cudaFree(R->d_g); cudaFree(R->d_f);
+    (void)cudaGetLastError();
+    delete R;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels, cbct_recon **out) {
+    if (!finest || !out || n_levels < 1 || n_levels > 8) return CBCT_E_INVALID;
+    *out = nullptr;
+    const int fac0 = 1 << (n_levels - 1);
+    if (finest->nx % fac0 || finest->ny % fac0) return CBCT_E_INVALID;   // x,y coarsened by 2 per level, z kept
+    cbct_recon *R = new (std::nothrow) cbct_recon();
+    if (!R) return CBCT_E_INVALID;
+    R->n_levels = n_levels;
+    R->d_r = R->d_g = R->d_f = nullptr;
+    R->n_rays = (int64_t)finest->nu * finest->nv * finest->n_views;
+    R->n_vox_finest = (int64_t)finest->nx * finest->ny * finest->nz;
+    int status = CBCT_OK;
+    for (int l = 0; l < n_levels && status == CBCT_OK; ++l) {
+        const int fac = 1 << (n_levels - 1 - l);
+        cbct_geometry_desc d = *finest;
+        d.nx = finest->nx / fac; d.ny = finest->ny / fac;
+        d.dx = finest->dx * fac; d.dy = finest->dy * fac;             // same extent, coarser pitch
+        cbct_recon_level L{};
+        L.nx = d.nx; L.ny = d.ny; L.nz = d.nz;
+        status = cbct_geometry_create(&d, &L.geom);
+        if (status == CBCT_OK) status = cbct_cgls_create(L.geom, &L.cg);
+        const size_t bytes = sizeof(float) * (size_t)d.nx * d.ny * d.nz;
+        float **bufs[5] = {&L.d_x, &L.d_p, &L.d_fa, &L.d_fb, &L.d_fc};
+        for (auto b : bufs)
+            if (status == CBCT_OK) {
+                cudaError_t e = cudaMalloc(b, bytes);
+                if (e != cudaSuccess) status = set_cuda_error(e);
+            }
+        R->lev.push_back(L);
+    }
+    float **pb[3] = {&R->d_r, &R->d_g, &R->d_f};
+    const size_t pbytes[3] = {sizeof(float) * (size_t)R->n_rays, sizeof(float) * (size_t)R->n_rays,
+                              sizeof(float) * (size_t)R->n_vox_finest};
+    for (int i = 0; i < 3 && status == CBCT_OK; ++i) {
+        cudaError_t e = cudaMalloc(pb[i], pbytes[i]);
+        if (e != cudaSuccess) status = set_cuda_error(e);
+    }
+    if (status != CBCT_OK) { cbct_recon_destroy(R); return status; }
+    *out = R;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_recon_run(cbct_recon *R, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu,
+                              int momentum, void *stream) {
+    if (!R || !d_g || !d_f || !n_outer || n_cgls < 0 || !(mu >= 0.f)) return CBCT_E_INVALID;
+    cudaStream_t st = as_stream(stream);
+    for (int l = 0; l < R->n_levels; ++l) {
+        cbct_recon_level &L = R->lev[l];
+        const int64_t n = (int64_t)L.nx * L.ny * L.nz;
+        float *f_cur = L.d_fa, *f_prev = L.d_fb, *f_new = L.d_fc;
+        if (l == 0) {
+            CBCT_CUDA_TRY(cudaMemsetAsync(f_cur, 0, sizeof(float) * n, st));          // f^(0) = 0
+        } else {
+            cbct_recon_level &C = R->lev[l - 1];                                         // "smoothly extend"
+            CBCT_TRY(mg_prolong(C.d_fa, f_cur, L.nx, L.ny, L.nz, 2, 2, 1, stream));
+        }
+        CBCT_CUDA_TRY(cudaMemcpyAsync(f_prev, f_cur, sizeof(float) * n, cudaMemcpyDeviceToDevice, st));  // f^(-1) = f^(0)
+        double t_prev = 1.0, t_cur = 1.0;                                                // t^(-1) = t^(0) = 1
+        for (int k = 0; k < n_outer[l]; ++k) {
+            const float coef = momentum ? (float)((t_prev - 1.0) / t_cur) : 0.f;
+            CBCT_TRY(cbct_a2_extrapolate(f_cur, f_prev, L.d_x, coef, n, stream));        // 1. v
+            CBCT_TRY(cbct_cgls_init(L.cg, d_g, L.d_x, R->d_r, L.d_p, stream));           // 2. f = CGLS[v]
+            for (int m = 0; m < n_cgls; ++m) CBCT_TRY(cbct_cgls_step(L.cg, L.d_x, R->d_r, L.d_p, stream));
+            CBCT_TRY(tf_apply_fused(L.d_x, f_new, mu, 1, L.nx, L.ny, L.nz, stream));     // 3.+4. shrink, clamp
+            float *tmp = f_prev; f_prev = f_cur; f_cur = f_new; f_new = tmp;
+            const double t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t_cur * t_cur));    // 5.
+            t_prev = t_cur; t_cur = t_next;
+        }
+        if (f_cur != L.d_fa)   // keep the level's result in d_fa for the prolongation / output
+            CBCT_CUDA_TRY(cudaMemcpyAsync(L.d_fa, f_cur, sizeof(float) * n, cudaMemcpyDeviceToDevice, st));
+    }
+    CBCT_CUDA_TRY(cudaMemcpyAsync(d_f, R->lev.back().d_fa, sizeof(float) * R->n_vox_finest, cudaMemcpyDeviceToDevice, st));
+    return CBCT_OK;
+}
+
+extern "C" int cbct_recon_run_host(cbct_recon *R, const float *h_g, float *h_f, const int *n_outer, int n_cgls, float mu,
+                                   int momentum, void *stream) {
+    if (!R || !h_g || !h_f) return CBCT_E_INVALID;
+    cudaStream_t st = as_stream(stream);
+    CBCT_CUDA_TRY(cudaMemcpyAsync(R->d_g, h_g, sizeof(float) * R->n_rays, cudaMemcpyHostToDevice, st));
+    CBCT_TRY(cbct_recon_run(R, R->d_g, R->d_f, n_outer, n_cgls, mu, momentum, stream));
+    CBCT_CUDA_TRY(cudaMemcpyAsync(h_f, R->d_f, sizeof(float) * R->n_vox_finest, cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA_TRY(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
+
+extern "C" int cbct_tf_reconstruct(const cbct_geometry_desc *finest, const float *d_g, float *d_f, int n_levels,
+                                   const int *n_outer, int n_cgls, float mu, int momentum, void *stream) {
+    cbct_recon *R = nullptr;
+    CBCT_TRY(cbct_recon_create(finest, n_levels, &R));
+    int s = cbct_recon_run(R, d_g, d_f, n_outer, n_cgls, mu, momentum, stream);
+    if (s == CBCT_OK) {
+        const cudaError_t e = cudaStreamSynchronize(as_stream(stream));
+        if (e != cudaSuccess) s = set_cuda_error(e);
+    }
+    cbct_recon_destroy(R);
+    return s;
+}
+
+extern "C" int cbct_tf_reconstruct_host(const cbct_geometry_desc *finest, const float *h_g, float *h_f, int n_levels,
+                                        const int *n_outer, int n_cgls, float mu, int momentum, void *stream) {
+    cbct_recon *R = nullptr;
+    CBCT_TRY(cbct_recon_create(finest, n_levels, &R));
+    const int s = cbct_recon_run_host(R, h_g, h_f, n_outer, n_cgls, mu, momentum, stream);
+    cbct_recon_destroy(R);
+    return s;
+}

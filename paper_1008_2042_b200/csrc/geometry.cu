@@ -1,0 +1,207 @@
+// geometry.cu -- status plumbing, geometry handle, host-buffer entry points.
+// cbct_geometry_create / _info: include/cbct.h; conventions of SURVEY.md §8(c) c.1-c.2.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+namespace cbct {
+
+static thread_local int g_last_cuda_error = 0;
+
+int set_cuda_error(cudaError_t e) {
+    g_last_cuda_error = (int)e;
+    (void)cudaGetLastError();  // clear the sticky-free error state
+    return CBCT_E_CUDA;
+}
+
+int device_supported() {
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return CBCT_E_UNSUPPORTED; }
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return CBCT_E_UNSUPPORTED;
+    }
+    return major == 10 ? CBCT_OK : CBCT_E_UNSUPPORTED;  // sm_100a code only: no other backend, no CPU path
+}
+
+// chord of every ray through the zero-padded box [-1, n]^3 (index space), in samples; block partials
+__global__ void sample_count_kernel(DevGeom g, double *partials) {
+    const long long n_rays = (long long)g.n_views * g.nv * g.nu;
+    double acc = 0.0;
+    for (long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x; r < n_rays;
+         r += (long long)gridDim.x * blockDim.x) {
+        const int iu = (int)(r % g.nu), iv = (int)((r / g.nu) % g.nv), view = (int)(r / ((long long)g.nu * g.nv));
+        RayF rf;
+        double b[3], c[3];
+        ray_setup(g, view, iv, iu, rf, b[0], b[1], b[2], c[0], c[1], c[2]);
+        const double hi[3] = {(double)g.nx, (double)g.ny, (double)g.nz};
+        double tin = -1e300, tout = 1e300;
+        bool miss = false;
+        for (int a = 0; a < 3; ++a) {
+            if (b[a] == 0.0) { miss |= (c[a] < -1.0 || c[a] > hi[a]); continue; }
+            double t1 = (-1.0 - c[a]) / b[a], t2 = (hi[a] - c[a]) / b[a];
+            if (t1 > t2) { double t = t1; t1 = t2; t2 = t; }
+            tin = fmax(tin, t1); tout = fmin(tout, t2);
+        }
+        if (!miss && tout > tin) acc += (tout - tin) / g.step;
+    }
+    __shared__ double sh[256];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partials[blockIdx.x] = sh[0];
+}
+
+}  // namespace cbct
+
+using namespace cbct;
+
+extern "C" const char *cbct_status_string(int status) {
+    switch (status) {
+        case CBCT_OK: return "ok";
+        case CBCT_E_INVALID: return "invalid argument";
+        case CBCT_E_UNSUPPORTED: return "unsupported device (needs compute capability 10.x, sm_100a)";
+        case CBCT_E_CUDA: return "CUDA runtime error (see cbct_last_cuda_error)";
+        case CBCT_BREAKDOWN: return "CGLS breakdown (gamma == 0 or ||q||^2 == 0)";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int cbct_last_cuda_error(void) { return g_last_cuda_error; }
+extern "C" int cbct_version(void) { return 100; }
+
+static int validate(const cbct_geometry_desc *d, double *R_out, double *step_out) {
+    if (!d || !d->angles) return CBCT_E_INVALID;
+    if (d->nx <= 0 || d->ny <= 0 || d->nz <= 0 || d->nu <= 0 || d->nv <= 0 || d->n_views <= 0) return CBCT_E_INVALID;
+    if (!(d->dx > 0) || !(d->dy > 0) || !(d->dz > 0) || !(d->du > 0) || !(d->dv > 0)) return CBCT_E_INVALID;
+    if (!(d->sad > 0) || !(d->sdd > d->sad)) return CBCT_E_INVALID;
+    if ((long long)d->nx * d->ny * d->nz > (1LL << 31) - 1) return CBCT_E_INVALID;
+    if ((long long)d->nu * d->nv * d->n_views > (1LL << 31) - 1) return CBCT_E_INVALID;
+    const double hx = 0.5 * (d->nx + 1) * d->dx, hy = 0.5 * (d->ny + 1) * d->dy, hz = 0.5 * (d->nz + 1) * d->dz;
+    const double R = std::sqrt(hx * hx + hy * hy + hz * hz) + std::sqrt(d->ox * d->ox + d->oy * d->oy + d->oz * d->oz);
+    if (!(R < d->sad)) return CBCT_E_INVALID;   // source would sit inside the padded volume
+    double step = d->step_mm > 0 ? d->step_mm : 0.5 * std::fmin(d->dx, std::fmin(d->dy, d->dz));
+    if (!(step > 0) || !std::isfinite(step)) return CBCT_E_INVALID;
+    if (2.0 * R / step > 1e7) return CBCT_E_INVALID;   // K must stay exactly representable in fp32
+    for (int i = 0; i < d->n_views; ++i)
+        if (!std::isfinite(d->angles[i])) return CBCT_E_INVALID;
+    *R_out = R;
+    *step_out = step;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometry **out) {
+    if (!out) return CBCT_E_INVALID;
+    *out = nullptr;
+    double R = 0, step = 0;
+    CBCT_TRY(validate(desc, &R, &step));
+    CBCT_TRY(device_supported());
+    cbct_geometry *G = new (std::nothrow) cbct_geometry();
+    if (!G) return CBCT_E_INVALID;
+    G->desc = *desc;
+    G->angles.assign(desc->angles, desc->angles + desc->n_views);
+    G->desc.angles = G->angles.data();
+    G->desc.step_mm = step;
+    G->R = R; G->step = step; G->t_min = desc->sad - R;
+    G->K = (int32_t)std::ceil(2.0 * R / step);
+    G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
+    G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
+    G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr;
+    G->workspace_bytes = 0;
+
+    std::vector<double2> cs(desc->n_views);
+    for (int i = 0; i < desc->n_views; ++i) cs[i] = make_double2(std::cos(desc->angles[i]), std::sin(desc->angles[i]));
+    cudaError_t e = cudaMalloc(&G->d_view_cs, sizeof(double2) * cs.size());
+    if (e == cudaSuccess) e = cudaMemcpy(G->d_view_cs, cs.data(), sizeof(double2) * cs.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&G->d_ws_vol, sizeof(float) * G->n_vox);
+    if (e == cudaSuccess) e = cudaMalloc(&G->d_ws_proj, sizeof(float) * G->n_rays);
+    if (e != cudaSuccess) { cbct_geometry_destroy(G); return set_cuda_error(e); }
+    G->workspace_bytes = sizeof(double2) * cs.size() + sizeof(float) * (G->n_vox + G->n_rays);
+
+    DevGeom &g = G->dg;
+    g.nx = desc->nx; g.ny = desc->ny; g.nz = desc->nz; g.nu = desc->nu; g.nv = desc->nv;
+    g.n_views = desc->n_views; g.K = G->K;
+    g.sad = desc->sad; g.sdd = desc->sdd; g.du = desc->du; g.dv = desc->dv;
+    g.u_first = desc->u0 - 0.5 * (desc->nu - 1) * desc->du;
+    g.v_first = desc->v0 - 0.5 * (desc->nv - 1) * desc->dv;
+    g.inv_dx = 1.0 / desc->dx; g.inv_dy = 1.0 / desc->dy; g.inv_dz = 1.0 / desc->dz;
+    g.cx = -desc->ox / desc->dx + 0.5 * (desc->nx - 1);
+    g.cy = -desc->oy / desc->dy + 0.5 * (desc->ny - 1);
+    g.cz = -desc->oz / desc->dz + 0.5 * (desc->nz - 1);
+    g.step = step;
+    g.tau0 = G->t_min + 0.5 * step - desc->sad;
+    g.view_cs = G->d_view_cs;
+
+    // algorithmic sample count (unit of Gsamples/s), once, on the device
+    const int blocks = 592;
+    double *d_part = nullptr;
+    e = cudaMalloc(&d_part, sizeof(double) * blocks);
+    if (e != cudaSuccess) { cbct_geometry_destroy(G); return set_cuda_error(e); }
+    sample_count_kernel<<<blocks, 256>>>(g, d_part);
+    std::vector<double> part(blocks);
+    e = cudaMemcpy(part.data(), d_part, sizeof(double) * blocks, cudaMemcpyDeviceToHost);
+    cudaFree(d_part);
+    if (e != cudaSuccess) { cbct_geometry_destroy(G); return set_cuda_error(e); }
+    double total = 0;
+    for (double p : part) total += p;
+    G->n_samples = (int64_t)std::llround(total);
+    *out = G;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
+    if (!G) return CBCT_OK;
+    cudaFree(G->d_view_cs);
+    cudaFree(G->d_ws_vol);
+    cudaFree(G->d_ws_proj);
+    cudaFree(G->d_bp_partial);
+    (void)cudaGetLastError();
+    delete G;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_geometry_info(const cbct_geometry *G, int64_t *n_vox, int64_t *n_rays, int32_t *K, double *t_min,
+                                  double *step_mm, int64_t *n_samples_algorithmic, size_t *workspace_bytes) {
+    if (!G) return CBCT_E_INVALID;
+    if (n_vox) *n_vox = G->n_vox;
+    if (n_rays) *n_rays = G->n_rays;
+    if (K) *K = G->K;
+    if (t_min) *t_min = G->t_min;
+    if (step_mm) *step_mm = G->step;
+    if (n_samples_algorithmic) *n_samples_algorithmic = G->n_samples;
+    if (workspace_bytes) *workspace_bytes = G->workspace_bytes;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, void *stream) {
+    if (!G || !d_vol || !d_proj) return CBCT_E_INVALID;
+    return launch_forward(G, d_vol, d_proj, as_stream(stream));
+}
+
+extern "C" int cbct_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, void *stream) {
+    if (!G || !d_vol || !d_proj) return CBCT_E_INVALID;
+    return launch_backproject(G, d_proj, d_vol, as_stream(stream));
+}
+
+extern "C" int cbct_forward_host(cbct_geometry *G, const float *h_vol, float *h_proj, void *stream) {
+    if (!G || !h_vol || !h_proj) return CBCT_E_INVALID;
+    cudaStream_t st = as_stream(stream);
+    CBCT_CUDA_TRY(cudaMemcpyAsync(G->d_ws_vol, h_vol, sizeof(float) * G->n_vox, cudaMemcpyHostToDevice, st));
+    CBCT_TRY(launch_forward(G, G->d_ws_vol, G->d_ws_proj, st));
+    CBCT_CUDA_TRY(cudaMemcpyAsync(h_proj, G->d_ws_proj, sizeof(float) * G->n_rays, cudaMemcpyDeviceToHost, st));
+    return CBCT_OK;
+}
+
+extern "C" int cbct_backproject_host(cbct_geometry *G, const float *h_proj, float *h_vol, void *stream) {
+    if (!G || !h_vol || !h_proj) return CBCT_E_INVALID;
+    cudaStream_t st = as_stream(stream);
+    CBCT_CUDA_TRY(cudaMemcpyAsync(G->d_ws_proj, h_proj, sizeof(float) * G->n_rays, cudaMemcpyHostToDevice, st));
+    CBCT_TRY(launch_backproject(G, G->d_ws_proj, G->d_ws_vol, st));
+    CBCT_CUDA_TRY(cudaMemcpyAsync(h_vol, G->d_ws_vol, sizeof(float) * G->n_vox, cudaMemcpyDeviceToHost, st));
+    return CBCT_OK;
+}

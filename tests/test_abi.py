@@ -1,0 +1,103 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol that
+include/cbct.h declares; argument validation that happens before any CUDA call; the binding fails
+loudly without the library."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1008_2042_b200 import binding, build
+from paper_1008_2042_b200 import synthetic as syn
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "cbct.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    names = re.findall(r"\b(?:int|const char \*)\s*\*?\s*((?:cbct|tf|mg)_\w+)\s*\(", text)
+    return sorted(set(names))
+
+
+@pytest.fixture(scope="module")
+def cdll():
+    path = build.build()
+    return ctypes.CDLL(path)
+
+
+def test_header_symbols_are_exported(cdll):
+    names = declared_symbols()
+    assert len(names) >= 25
+    for n in names:
+        assert hasattr(cdll, n), f"{n} declared in include/cbct.h but not exported"
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_status_strings_and_version(cdll):
+    cdll.cbct_status_string.restype = ctypes.c_char_p
+    assert cdll.cbct_status_string(0) == b"ok"
+    for code in (-1, -2, -3, 1):
+        assert len(cdll.cbct_status_string(code)) > 3
+    assert cdll.cbct_version() >= 100
+    assert cdll.cbct_last_cuda_error() == 0
+
+
+def test_invalid_arguments_rejected_before_any_cuda_call():
+    L = binding.lib()
+    G = syn.workload(1).geometry
+    out = ctypes.c_void_p()
+    assert L.cbct_geometry_create(None, ctypes.byref(out)) == binding.CBCT_E_INVALID
+    bad = [dict(nx=0), dict(dx=-1.0), dict(sdd=900.0), dict(sad=-5.0), dict(nu=0), dict(sad=100.0, sdd=150.0)]
+    from dataclasses import replace
+    for kw in bad:
+        d, keep = binding.make_desc(replace(G, **kw))
+        assert L.cbct_geometry_create(ctypes.byref(d), ctypes.byref(out)) == binding.CBCT_E_INVALID, kw
+    d, keep = binding.make_desc(G)
+    d.angles = None
+    assert L.cbct_geometry_create(ctypes.byref(d), ctypes.byref(out)) == binding.CBCT_E_INVALID
+    assert L.cbct_forward(None, None, None, None) == binding.CBCT_E_INVALID
+    assert L.tf_decompose(None, None, 4, 4, 4, None) == binding.CBCT_E_INVALID
+    assert L.mg_restrict(1, 1, 5, 4, 4, 2, 2, 1, None) == binding.CBCT_E_INVALID     # 5 not divisible by 2
+    assert L.mg_prolong(1, 1, 4, 4, 4, 3, 1, 1, None) == binding.CBCT_E_INVALID      # factor not in {1,2}
+    assert L.cbct_recon_create(ctypes.byref(binding.make_desc(G)[0]), 0, ctypes.byref(out)) == binding.CBCT_E_INVALID
+
+
+def test_no_cpu_fallback_without_a_device():
+    """On a box without an sm_100 GPU the product path must refuse, not fall back."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    d, keep = binding.make_desc(syn.workload(1).geometry)
+    out = ctypes.c_void_p()
+    assert binding.lib().cbct_geometry_create(ctypes.byref(d), ctypes.byref(out)) == binding.CBCT_E_UNSUPPORTED
+    with pytest.raises(binding.CbctError):
+        binding.Geometry(syn.workload(1).geometry)
+
+
+def test_product_path_does_not_import_the_oracle():
+    for root, _dirs, files in os.walk(os.path.join(ROOT, "paper_1008_2042_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(root, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text and "cbct_oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_1008_2042_b200", text, flags=re.M), f
+            assert "csrc/" not in text.replace("paper_1008_2042_b200/csrc)", ""), f
+
+
+def test_synthetic_workloads_match_baseline_configs():
+    shapes = {1: ((16, 64, 64), (32, 32, 96)), 2: ((32, 128, 128), (40, 96, 256)), 3: ((70, 256, 256), (40, 384, 512)),
+              4: ((70, 512, 512), (40, 384, 512)), 5: ((70, 512, 512), (360, 768, 1024))}
+    for i, (vs, ps) in shapes.items():
+        w = syn.workload(i)
+        assert w.geometry.vol_shape == vs and w.geometry.proj_shape == ps
+        assert w.geometry.sad == 1000.0 and w.geometry.sdd == 1500.0
+    w, ells, f0, g = syn.make_inputs(1)
+    assert f0.dtype == np.float32 and g.dtype == np.float32 and len(ells) == 6
+    assert f0.max() > 0 and g.max() > 0
+    w2, _, f2, g2 = syn.make_inputs(1)
+    assert np.array_equal(f0, f2) and np.array_equal(g, g2)          # seeded

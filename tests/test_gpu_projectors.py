@@ -1,0 +1,174 @@
+"""GPU parity of P and P^T against the fp64 oracle, through the C ABI (python -m pytest -m gpu).
+
+Tolerances (BASELINE.json north_star): relative L2 <= 1e-5 per projection view and per backprojected
+volume; adjoint identity <= 1e-5 in fp32.  SURVEY.md §8(c) item 29 defines the norm.
+"""
+import math
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import projector as op                      # noqa: E402
+from paper_1008_2042_b200 import binding as cb          # noqa: E402
+from paper_1008_2042_b200 import synthetic as syn       # noqa: E402
+
+TOL = 1e-5
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def rel_l2_per_view(g, ref):
+    num = np.sqrt(np.sum((g.astype(np.float64) - ref) ** 2, axis=(1, 2)))
+    den = np.sqrt(np.sum(ref ** 2, axis=(1, 2)))
+    scale = np.max(np.abs(ref))
+    return np.max(np.where(den > 0, num / np.where(den > 0, den, 1.0), num / (scale if scale > 0 else 1.0)))
+
+
+def rel_l2(a, ref):
+    return float(np.linalg.norm(a.astype(np.float64).ravel() - ref.ravel()) / np.linalg.norm(ref.ravel()))
+
+
+def gpu_forward(G, f):
+    h = cb.Geometry(G)
+    out = torch.empty(h.proj_shape, dtype=torch.float32, device="cuda")
+    h.forward(dev(f), out)
+    torch.cuda.synchronize()
+    return out.cpu().numpy(), h
+
+
+def gpu_back(G, g):
+    h = cb.Geometry(G)
+    out = torch.empty(h.vol_shape, dtype=torch.float32, device="cuda")
+    h.backproject(dev(g), out)
+    torch.cuda.synchronize()
+    return out.cpu().numpy(), h
+
+
+ODD = syn.Geometry(37, 29, 11, 2.0, 3.0, 5.0, 45, 19, 2.3, 3.1, 1000.0, 1500.0,
+                   (0.0, 0.4, math.pi / 4, math.pi / 2, 2.0, math.pi, 4.0, 5.5), ox=3.0, oy=-4.0, oz=2.0, u0=1.7, v0=-2.9,
+                   step_mm=0.7)
+
+
+def test_geometry_info_matches_oracle_grid():
+    for idx in (1, 2):
+        G = syn.workload(idx).geometry
+        h = cb.Geometry(G)
+        R, t_min, K = op.grid(G)
+        assert h.K == K and abs(h.t_min - t_min) < 1e-9 and abs(h.step_mm - G.step) < 1e-12
+        assert h.n_vox == G.nx * G.ny * G.nz and h.n_rays == G.n_views * G.nv * G.nu
+        assert abs(h.n_samples - op.sample_count(G)) <= 1e-9 * h.n_samples + 1
+        assert h.workspace_bytes > 0
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_forward_matches_oracle_full(cfg):
+    w, ells, f0, _ = syn.make_inputs(cfg, noisy=False)
+    g, h = gpu_forward(w.geometry, f0)
+    ref = op.forward(w.geometry, f0.astype(np.float64))
+    assert rel_l2_per_view(g, ref) <= TOL
+
+
+def test_forward_ragged_offset_geometry():
+    f = syn.uniform_volume(ODD, 21)
+    g, _ = gpu_forward(ODD, f)
+    ref = op.forward(ODD, f.astype(np.float64))
+    assert rel_l2_per_view(g, ref) <= TOL
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_backproject_matches_oracle_full(cfg):
+    G = syn.workload(cfg).geometry
+    y = syn.uniform_projections(G, 31)
+    f, _ = gpu_back(G, y)
+    ref = op.back_scatter(G, y.astype(np.float64))
+    assert rel_l2(f, ref) <= TOL
+
+
+def test_backproject_ragged_offset_geometry():
+    y = syn.uniform_projections(ODD, 22) - 0.3
+    f, _ = gpu_back(ODD, y)
+    ref = op.back_scatter(ODD, y.astype(np.float64))
+    assert rel_l2(f, ref) <= TOL
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_adjoint_identity_fp32(cfg):
+    """<P x, y> = <x, P^T y> to 1e-5 with U[0,1) vectors, inner products accumulated in fp64."""
+    G = syn.workload(cfg).geometry
+    x, y = syn.uniform_volume(G, 41), syn.uniform_projections(G, 41)
+    Px, _ = gpu_forward(G, x)
+    PTy, _ = gpu_back(G, y)
+    lhs = float(np.sum(Px.astype(np.float64) * y))
+    rhs = float(np.sum(x.astype(np.float64) * PTy))
+    assert abs(lhs - rhs) <= TOL * abs(lhs)
+
+
+def test_degenerate_inputs():
+    G = syn.workload(1).geometry
+    g, _ = gpu_forward(G, np.zeros(G.vol_shape, np.float32))
+    assert np.all(g == 0.0)
+    f, _ = gpu_back(G, np.zeros(G.proj_shape, np.float32))
+    assert np.all(f == 0.0)
+    # detector entirely beside the volume: every ray misses -> exact zeros, and P^T of anything is zero
+    Gm = replace(G, u0=5000.0)
+    g, _ = gpu_forward(Gm, syn.uniform_volume(Gm, 1))
+    assert np.all(g == 0.0)
+    f, _ = gpu_back(Gm, syn.uniform_projections(Gm, 1))
+    assert np.all(f == 0.0)
+    # single voxel, single pixel, single view
+    G1 = syn.Geometry(1, 1, 1, 4.0, 4.0, 4.0, 1, 1, 1.0, 1.0, 1000.0, 1500.0, (0.3,))
+    g, _ = gpu_forward(G1, np.ones((1, 1, 1), np.float32))
+    ref = op.forward(G1, np.ones((1, 1, 1)))
+    assert abs(g[0, 0, 0] - ref[0, 0, 0]) <= TOL * ref[0, 0, 0]
+    f, _ = gpu_back(G1, np.ones((1, 1, 1), np.float32))
+    assert abs(f[0, 0, 0] - op.back_scatter(G1, np.ones((1, 1, 1)))[0, 0, 0]) <= TOL * f[0, 0, 0]
+
+
+def test_host_buffer_entry_points_match_device_ones():
+    G = syn.workload(1).geometry
+    h = cb.Geometry(G)
+    x, y = syn.uniform_volume(G, 51), syn.uniform_projections(G, 51)
+    hx, hy = torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()
+    out_g = torch.empty(h.proj_shape, dtype=torch.float32).pin_memory()
+    out_f = torch.empty(h.vol_shape, dtype=torch.float32).pin_memory()
+    h.forward_host(hx, out_g)
+    h.backproject_host(hy, out_f)
+    torch.cuda.synchronize()
+    g, _ = gpu_forward(G, x)
+    f, _ = gpu_back(G, y)
+    assert np.array_equal(out_g.numpy(), g) and np.array_equal(out_f.numpy(), f)
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_sampled_outputs(cfg):
+    """BASELINE sizes in the launch configuration bench.py times: oracle on sampled rays / voxels."""
+    w = syn.workload(cfg)
+    G = w.geometry
+    f0 = syn.voxelise(G, syn.ellipsoids_for(w))
+    g, h = gpu_forward(G, f0)
+    rng = np.random.default_rng(cfg)
+    rays = np.sort(rng.choice(h.n_rays, 4000, replace=False))
+    ref = op.forward_rays(G, f0.astype(np.float64), rays)
+    got = g.ravel()[rays].astype(np.float64)
+    assert np.linalg.norm(got - ref) <= TOL * np.linalg.norm(ref)
+    assert np.max(np.abs(got - ref)) <= 2e-5 * np.max(np.abs(ref))
+    y = syn.uniform_projections(G, cfg)
+    f, _ = gpu_back(G, y)
+    vox = np.sort(rng.choice(h.n_vox, 300, replace=False))
+    vox[:4] = [0, G.nx - 1, h.n_vox - G.nx, h.n_vox - 1]                 # the four extreme corners too
+    refv = op.back_gather_voxels(G, y.astype(np.float64), vox)
+    gotv = f.ravel()[vox].astype(np.float64)
+    assert np.linalg.norm(gotv - refv) <= TOL * np.linalg.norm(refv)
+    # property that holds at any size: adjoint identity
+    x = syn.uniform_volume(G, cfg)
+    Px, _ = gpu_forward(G, x)
+    lhs = float(np.sum(Px.astype(np.float64) * y))
+    rhs = float(np.sum(x.astype(np.float64) * f))
+    assert abs(lhs - rhs) <= TOL * abs(lhs)
