@@ -43,6 +43,13 @@ const char *cbct_status_string(int status);
 int cbct_last_cuda_error(void);
 /* Library version, e.g. 100 = 1.0.0. */
 int cbct_version(void);
+/* Number of kernels of this library launched by this process so far (all threads). */
+long long cbct_launch_count(void);
+/* Optional kernel timer.  Between _begin and _end every cbct_forward / cbct_backproject launch (also
+ * those inside CGLS and the driver) is bracketed by CUDA events on its own stream.  _end waits for
+ * those events and returns the summed device time in ms and the launch count, index 0 = P, 1 = P^T. */
+int cbct_profile_begin(void);
+int cbct_profile_end(double ms[2], int count[2]);
 
 /* ------------------------------------------------------------------------------------------------
  * Geometry: circular orbit, flat panel (Eq. 1, Fig. 1 caption).

@@ -19,7 +19,8 @@ CBCT_OK, CBCT_E_INVALID, CBCT_E_UNSUPPORTED, CBCT_E_CUDA, CBCT_BREAKDOWN = 0, -1
 
 # every symbol include/cbct.h declares (tests check the library exports all of them)
 EXPORTS = [
-    "cbct_status_string", "cbct_last_cuda_error", "cbct_version",
+    "cbct_status_string", "cbct_last_cuda_error", "cbct_version", "cbct_launch_count",
+    "cbct_profile_begin", "cbct_profile_end",
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
@@ -66,6 +67,9 @@ def lib():
     L.cbct_status_string.argtypes = [ip]
     L.cbct_last_cuda_error.argtypes = []
     L.cbct_version.argtypes = []
+    L.cbct_launch_count.argtypes = []
+    L.cbct_profile_begin.argtypes = []
+    L.cbct_profile_end.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int)]
     L.cbct_geometry_create.argtypes = [C.POINTER(GeometryDesc), C.POINTER(vp)]
     L.cbct_geometry_destroy.argtypes = [vp]
     L.cbct_geometry_info.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32),
@@ -94,6 +98,7 @@ def lib():
     for name in EXPORTS:
         if name != "cbct_status_string":
             getattr(L, name).restype = C.c_int
+    L.cbct_launch_count.restype = C.c_longlong
     _lib = L
     return L
 
@@ -102,6 +107,21 @@ def _check(status: int, where: str, allow_breakdown: bool = False) -> int:
     if status == CBCT_OK or (allow_breakdown and status == CBCT_BREAKDOWN):
         return status
     raise CbctError(status, where)
+
+
+def launch_count() -> int:
+    return int(lib().cbct_launch_count())
+
+
+def profile_begin() -> None:
+    _check(lib().cbct_profile_begin(), "cbct_profile_begin")
+
+
+def profile_end():
+    """{'forward': (ms, launches), 'backproject': (ms, launches)} since profile_begin()."""
+    ms, cnt = (C.c_double * 2)(), (C.c_int * 2)()
+    _check(lib().cbct_profile_end(ms, cnt), "cbct_profile_end")
+    return {"forward": (ms[0], cnt[0]), "backproject": (ms[1], cnt[1])}
 
 
 def _stream(stream=None) -> int:

@@ -81,6 +81,7 @@ __global__ void __launch_bounds__(128) backproject_gather_kernel(DevGeom g, cons
 
 int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
     const DevGeom &g = G->dg;
+    ProfScope prof(PROF_BACK, st);
     dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4), g.nz);
     backproject_gather_kernel<<<grid, block, 0, st>>>(g, d_proj, d_vol);
     CBCT_LAUNCH_CHECK();

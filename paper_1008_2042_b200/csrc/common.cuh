@@ -22,7 +22,21 @@ int device_supported();                     // CBCT_OK on a compute-capability-1
         int _s = (expr);               \
         if (_s != CBCT_OK) return _s;  \
     } while (0)
-#define CBCT_LAUNCH_CHECK() CBCT_CUDA_TRY(cudaGetLastError())
+void count_launch();                        // one of OUR kernels was launched (cbct_launch_count)
+#define CBCT_LAUNCH_CHECK()                   \
+    do {                                      \
+        ::cbct::count_launch();               \
+        CBCT_CUDA_TRY(cudaGetLastError());    \
+    } while (0)
+
+// optional in-library kernel timer: CUDA events recorded on the launching stream around P / P^T
+enum { PROF_FORWARD = 0, PROF_BACK = 1, PROF_KINDS = 2 };
+struct ProfScope {
+    int slot;
+    cudaStream_t st;
+    ProfScope(int kind, cudaStream_t s);
+    ~ProfScope();
+};
 
 static inline cudaStream_t as_stream(void *s) { return reinterpret_cast<cudaStream_t>(s); }
 static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }

@@ -74,6 +74,7 @@ __global__ void __launch_bounds__(256) forward_global_kernel(DevGeom g, const fl
 
 int launch_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st) {
     const DevGeom &g = G->dg;
+    ProfScope prof(PROF_FORWARD, st);
     dim3 block(32, 8), grid(cdiv(g.nu, 32), cdiv(g.nv, 8), g.n_views);
     forward_global_kernel<<<grid, block, 0, st>>>(g, d_vol, d_proj);
     CBCT_LAUNCH_CHECK();

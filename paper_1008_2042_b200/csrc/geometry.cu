@@ -1,7 +1,9 @@
 // geometry.cu -- status plumbing, geometry handle, host-buffer entry points.
 // cbct_geometry_create / _info: include/cbct.h; conventions of SURVEY.md §8(c) c.1-c.2.
+#include <atomic>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "common.cuh"
@@ -14,6 +16,31 @@ int set_cuda_error(cudaError_t e) {
     g_last_cuda_error = (int)e;
     (void)cudaGetLastError();  // clear the sticky-free error state
     return CBCT_E_CUDA;
+}
+
+static std::atomic<long long> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+// ---- kernel timer ----------------------------------------------------------------------------
+static std::mutex g_prof_mu;
+static bool g_prof_on = false;
+struct ProfRec { cudaEvent_t a, b; int kind; };
+static std::vector<ProfRec> g_prof;
+
+ProfScope::ProfScope(int kind, cudaStream_t s) : slot(-1), st(s) {
+    if (!g_prof_on) return;
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    ProfRec r{};
+    r.kind = kind;
+    if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) { (void)cudaGetLastError(); return; }
+    cudaEventRecord(r.a, st);
+    g_prof.push_back(r);
+    slot = (int)g_prof.size() - 1;
+}
+ProfScope::~ProfScope() {
+    if (slot < 0) return;
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    cudaEventRecord(g_prof[slot].b, st);
 }
 
 int device_supported() {
@@ -74,6 +101,32 @@ extern "C" const char *cbct_status_string(int status) {
 
 extern "C" int cbct_last_cuda_error(void) { return g_last_cuda_error; }
 extern "C" int cbct_version(void) { return 100; }
+extern "C" long long cbct_launch_count(void) { return g_launches.load(); }
+
+extern "C" int cbct_profile_begin(void) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    for (auto &r : g_prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    g_prof.clear();
+    g_prof_on = true;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_profile_end(double ms[2], int count[2]) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_prof_on = false;
+    int status = CBCT_OK;
+    for (int k = 0; k < PROF_KINDS; ++k) { if (ms) ms[k] = 0.0; if (count) count[k] = 0; }
+    for (auto &r : g_prof) {
+        float t = 0.f;
+        cudaError_t e = cudaEventSynchronize(r.b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.a, r.b);
+        if (e != cudaSuccess) status = set_cuda_error(e);
+        else { if (ms) ms[r.kind] += t; if (count) count[r.kind] += 1; }
+        cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+    }
+    g_prof.clear();
+    return status;
+}
 
 static int validate(const cbct_geometry_desc *d, double *R_out, double *step_out) {
     if (!d || !d->angles) return CBCT_E_INVALID;

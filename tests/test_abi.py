@@ -17,7 +17,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "cbct.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    names = re.findall(r"\b(?:int|const char \*)\s*\*?\s*((?:cbct|tf|mg)_\w+)\s*\(", text)
+    names = re.findall(r"\b(?:int|long long|const char \*)\s*\*?\s*((?:cbct|tf|mg)_\w+)\s*\(", text)
     return sorted(set(names))
 
 
