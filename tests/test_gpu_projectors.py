@@ -82,6 +82,23 @@ def test_forward_ragged_offset_geometry():
     assert rel_l2_per_view(g, ref) <= TOL
 
 
+def test_forward_global_kernel_and_oversized_tiles(monkeypatch):
+    """The untiled kernel (CBCT_FORWARD_IMPL=global) and geometries whose pixel tiles do not fit the
+    shared-memory box (fine voxels under coarse pixels) go through the same parity bar."""
+    f = syn.uniform_volume(ODD, 23)
+    ref = op.forward(ODD, f.astype(np.float64))
+    monkeypatch.setenv("CBCT_FORWARD_IMPL", "global")
+    g, _ = gpu_forward(ODD, f)
+    monkeypatch.delenv("CBCT_FORWARD_IMPL")
+    assert rel_l2_per_view(g, ref) <= TOL
+    for vox, pix in ((0.25, 3.0), (0.6, 2.0), (1.0, 1.2)):
+        G = syn.Geometry(96, 80, 24, vox, vox, 2 * vox, 40, 12, pix, pix, 1000.0, 1500.0, (0.1, 0.9, 2.4, 3.9),
+                         step_mm=0.8 * vox)
+        f = syn.uniform_volume(G, 24)
+        g, _ = gpu_forward(G, f)
+        assert rel_l2_per_view(g, op.forward(G, f.astype(np.float64))) <= TOL, (vox, pix)
+
+
 @pytest.mark.parametrize("cfg", [1, 2])
 def test_backproject_matches_oracle_full(cfg):
     G = syn.workload(cfg).geometry
