@@ -149,6 +149,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernels-only", action="store_true", help="run P, P^T, fused TF 3x and exit (for ncu)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -182,6 +183,28 @@ def main():
     g = syn.analytic_projections(G, ells)
     if w.photons:
         g = syn.add_poisson_noise(g, w.photons, w.seed + rank)          # every replica its own noise draw
+
+    if args.kernels_only:
+        # short command for `ncu --set full`: 3 x (P, P^T, fused TF) on the workload, nothing else
+        geom = cb.Geometry(G)
+        d_vol = torch.from_numpy(f0).cuda()
+        d_g = torch.from_numpy(g).cuda()
+        d_proj = torch.empty(geom.proj_shape, dtype=torch.float32, device="cuda")
+        d_out = torch.empty(geom.vol_shape, dtype=torch.float32, device="cuda")
+        evs = []
+        for _ in range(3):
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            e[0].record(); geom.forward(d_vol, d_proj)
+            e[1].record(); geom.backproject(d_g, d_out)
+            e[2].record(); cb.tf_apply_fused(d_vol, d_out, MU, True)
+            e[3].record()
+            evs.append(e)
+        torch.cuda.synchronize()
+        e = evs[-1]
+        print(json.dumps(dict(kernels_only=True, workload=args.workload, p_ms=e[0].elapsed_time(e[1]),
+                              pt_ms=e[1].elapsed_time(e[2]), tf_fused_ms=e[2].elapsed_time(e[3]),
+                              samples=geom.n_samples)), flush=True)
+        return
 
     geom = cb.Geometry(G)                                                 # for the standalone P / P^T timing
     rec = cb.Recon(G, 1)

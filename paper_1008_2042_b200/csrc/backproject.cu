@@ -4,6 +4,10 @@
 //   f_j = step * sum_rays g_ray * sum_k hat(X_k - jx) hat(Y_k - jy) hat(Z_k - jz)
 // (SURVEY.md §8(c) c.3).  No atomics: each output voxel is owned by one thread, so the result is
 // deterministic.
+#include <cmath>
+#include <cstdlib>
+#include <vector>
+
 #include "common.cuh"
 
 namespace cbct {
@@ -79,12 +83,207 @@ __global__ void __launch_bounds__(128) backproject_gather_kernel(DevGeom g, cons
     vol[((size_t)jz * g.ny + jy) * g.nx + jx] = total * stepf;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Cell-driven path (the one that normally runs).  Still output-stationary and atomic-free, but the unit
+// of ownership is a CELL (the cube between 8 neighbouring voxel centres, padding cells included): a
+// sample of the forward projector lies in exactly one cell and spreads to that cell's 8 corners with
+// the trilinear weights, so one thread per cell evaluates each sample ONCE (the transposed lerp tree,
+// 15 flops) instead of once per touched voxel (8 hat products).  A second kernel sums, for every
+// voxel, the 8 corner accumulators of the 8 cells around it in a fixed order.
+//   per (cell, view): candidate detector columns from the projected cell centre +- a bound,
+//   per column: clip against the cell's x,y slabs in r = t/L (independent of the detector row),
+//   per row: clip against the z slab, k-range of the global sample grid, then the samples.
+// A sample belongs to the cell iff floor(X,Y,Z) == (ix,iy,iz), evaluated on the same fp32 X,Y,Z in
+// every thread, so each sample is counted exactly once however the clipping rounds.
+// ------------------------------------------------------------------------------------------------
+constexpr float BP_EPS = 0.02f;
+
+__global__ void __launch_bounds__(128) backproject_cell_kernel(BpTables P, int nx, int ny, int nz, int nu, int nv,
+                                                               int n_views, int K, const float *__restrict__ proj,
+                                                               float *__restrict__ partial) {
+    const int ix = blockIdx.x * 32 + threadIdx.x - 1, iy = blockIdx.y * 4 + threadIdx.y - 1, iz = blockIdx.z - 1;
+    if (ix > nx - 1 || iy > ny - 1) return;
+    const float fix = (float)ix, fiy = (float)iy, fiz = (float)iz;
+    const float az = fiz - P.Kz, bz = az + 1.f;
+    float a000 = 0.f, a100 = 0.f, a010 = 0.f, a110 = 0.f, a001 = 0.f, a101 = 0.f, a011 = 0.f, a111 = 0.f;
+    for (int view = 0; view < n_views; ++view) {
+        const BpView V = P.views[view];
+        // candidate columns: projected cell centre +- conservative half width
+        const float D = fmaf(V.Dx, fix + 0.5f, fmaf(V.Dy, fiy + 0.5f, V.D0));
+        const float tc = fmaf(V.Tx, fix + 0.5f, fmaf(V.Ty, fiy + 0.5f, V.T0));
+        const float rD = __frcp_rn(D), rDn = __frcp_rn(D - V.hd);
+        const float uc = P.sdd * tc * rD;
+        const float dumax = P.sdd * rDn * fmaf(fabsf(tc) * rD, V.hd, V.hl);
+        const int iu0 = max(0, (int)ceilf((uc - dumax - P.u_first) * P.inv_du - BP_EPS));
+        const int iu1 = min(nu - 1, (int)floorf((uc + dumax - P.u_first) * P.inv_du + BP_EPS));
+        const BpViewU *vu = P.viewu + (size_t)view * nu;
+        const float *pv = proj + (size_t)view * nv * nu;
+        for (int iu = iu0; iu <= iu1; ++iu) {
+            const float4 w0 = __ldg(reinterpret_cast<const float4 *>(vu + iu));        // Ax Ay Wx Wy
+            const float rx0 = (fix - V.Kx) * w0.z, rx1 = rx0 + w0.z;
+            const float ry0 = (fiy - V.Ky) * w0.w, ry1 = ry0 + w0.w;
+            const float rin = fmaxf(fminf(rx0, rx1), fminf(ry0, ry1)), rout = fminf(fmaxf(rx0, rx1), fmaxf(ry0, ry1));
+            if (!(rin < rout) || !(rin > 0.f)) continue;
+            const float2 w1 = __ldg(reinterpret_cast<const float2 *>(vu + iu) + 2);    // Gx Gy
+            const float i_in = __frcp_rn(rin), i_out = __frcp_rn(rout);
+            const float vzmin = fminf(az * i_in, az * i_out), vzmax = fmaxf(bz * i_in, bz * i_out);
+            const int iv0 = max(0, (int)ceilf(fmaf(vzmin, P.dz_dv, -P.vfirst_dv) - BP_EPS));
+            const int iv1 = min(nv - 1, (int)floorf(fmaf(vzmax, P.dz_dv, -P.vfirst_dv) + BP_EPS));
+            for (int iv = iv0; iv <= iv1; ++iv) {
+                const float2 rw = __ldg(P.rows + iv);                                  // vz, 1/vz
+                const float rz0 = az * rw.y, rz1 = bz * rw.y;
+                const float rlo = fmaxf(rin, fminf(rz0, rz1)), rhi = fminf(rout, fmaxf(rz0, rz1));
+                if (!(rlo <= rhi)) continue;
+                const float4 t = __ldg(P.pix + (size_t)iv * nu + iu);                  // 1/L, q, L
+                const int ka = max(0, (int)ceilf(fmaf(rlo, t.z, -P.t0) * P.inv_step - P.k_eps));
+                const int kb = min(K - 1, (int)floorf(fmaf(rhi, t.z, -P.t0) * P.inv_step + P.k_eps));
+                if (ka > kb) continue;
+                const float gval = __ldg(pv + (size_t)iv * nu + iu);
+                const float bx = w0.x * t.x, by = w0.y * t.x, bzz = rw.x * t.x;
+                const float cx = fmaf(w1.x, t.x, fmaf(V.Fx, t.y, P.cx0));
+                const float cy = fmaf(w1.y, t.x, fmaf(V.Fy, t.y, P.cy0));
+                const float cz = fmaf(P.sad * rw.x, t.x, P.cz0);
+                for (int k = ka; k <= kb; ++k) {
+                    const float tau = fmaf((float)k, P.stepf, P.tau0f);
+                    // X,Y,Z depend on (view, iu, iv, k) only, so all cells agree on them; X - ix is exact
+                    const float fx = fmaf(bx, tau, cx) - fix, fy = fmaf(by, tau, cy) - fiy, fz = fmaf(bzz, tau, cz) - fiz;
+                    const bool in = fx >= 0.f && fx < 1.f && fy >= 0.f && fy < 1.f && fz >= 0.f && fz < 1.f;
+                    const float gg = in ? gval : 0.f;
+                    const float g1 = gg * fz, g0 = gg - g1;
+                    const float g01 = g0 * fy, g00 = g0 - g01, g11 = g1 * fy, g10 = g1 - g11;
+                    const float ofx = 1.f - fx;
+                    a000 = fmaf(g00, ofx, a000); a100 = fmaf(g00, fx, a100);
+                    a010 = fmaf(g01, ofx, a010); a110 = fmaf(g01, fx, a110);
+                    a001 = fmaf(g10, ofx, a001); a101 = fmaf(g10, fx, a101);
+                    a011 = fmaf(g11, ofx, a011); a111 = fmaf(g11, fx, a111);
+                }
+            }
+        }
+    }
+    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * (nz + 1);
+    const size_t ci = ((size_t)(iz + 1) * (ny + 1) + (iy + 1)) * (nx + 1) + (ix + 1);
+    partial[ci] = a000; partial[ncell + ci] = a100; partial[2 * ncell + ci] = a010; partial[3 * ncell + ci] = a110;
+    partial[4 * ncell + ci] = a001; partial[5 * ncell + ci] = a101; partial[6 * ncell + ci] = a011;
+    partial[7 * ncell + ci] = a111;
+}
+
+// voxel (x,y,z) = step * sum over the 8 cells (x-dx, y-dy, z-dz) of their corner (dx,dy,dz) accumulator
+__global__ void __launch_bounds__(256) backproject_combine_kernel(const float *__restrict__ partial, float *__restrict__ vol,
+                                                                  int nx, int ny, int nz, float stepf) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y * blockDim.y + threadIdx.y, z = blockIdx.z;
+    if (x >= nx || y >= ny) return;
+    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * (nz + 1);
+    float acc = 0.f;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const int dx = c & 1, dy = (c >> 1) & 1, dz = c >> 2;
+        const size_t ci = ((size_t)(z - dz + 1) * (ny + 1) + (y - dy + 1)) * (nx + 1) + (x - dx + 1);
+        acc += __ldg(partial + (size_t)c * ncell + ci);
+    }
+    vol[((size_t)z * ny + y) * nx + x] = acc * stepf;
+}
+
+void free_bp_tables(cbct_geometry *G) {
+    cudaFree(const_cast<BpView *>(G->bp.views));
+    cudaFree(const_cast<BpViewU *>(G->bp.viewu));
+    cudaFree(const_cast<float4 *>(G->bp.pix));
+    cudaFree(const_cast<float2 *>(G->bp.rows));
+    cudaFree(G->d_bp_partial);
+    G->bp = BpTables{};
+    G->d_bp_partial = nullptr;
+}
+
+static double nudge(double a, double floor_mag) {
+    if (std::fabs(a) >= floor_mag) return a;
+    return a < 0 ? -floor_mag : floor_mag;
+}
+
+int build_bp_tables(cbct_geometry *G) {
+    const cbct_geometry_desc &d = G->desc;
+    const int nu = d.nu, nv = d.nv, nvw = d.n_views;
+    std::vector<BpView> views(nvw);
+    std::vector<BpViewU> viewu((size_t)nvw * nu);
+    std::vector<float4> pix((size_t)nv * nu);
+    std::vector<float2> rows(nv);
+    const double cx0 = -d.ox / d.dx + 0.5 * (d.nx - 1), cy0 = -d.oy / d.dy + 0.5 * (d.ny - 1),
+                 cz0 = -d.oz / d.dz + 0.5 * (d.nz - 1);
+    const double u_first = d.u0 - 0.5 * (nu - 1) * d.du, v_first = d.v0 - 0.5 * (nv - 1) * d.dv;
+    for (int i = 0; i < nvw; ++i) {
+        const double c = std::cos(d.angles[i]), s = std::sin(d.angles[i]);
+        BpView &V = views[i];
+        V.Kx = (float)(d.sad * c / d.dx + cx0); V.Ky = (float)(d.sad * s / d.dy + cy0);
+        V.Fx = (float)(d.sad * c / d.dx); V.Fy = (float)(d.sad * s / d.dy);
+        // world x = (X - cx0) dx, y = (Y - cy0) dy
+        V.Dx = (float)(-c * d.dx); V.Dy = (float)(-s * d.dy);
+        V.D0 = (float)(d.sad + c * cx0 * d.dx + s * cy0 * d.dy);
+        V.Tx = (float)(-s * d.dx); V.Ty = (float)(c * d.dy);
+        V.T0 = (float)(s * cx0 * d.dx - c * cy0 * d.dy);
+        V.hl = (float)(0.5 * (std::fabs(s) * d.dx + std::fabs(c) * d.dy));
+        V.hd = (float)(0.5 * (std::fabs(c) * d.dx + std::fabs(s) * d.dy));
+        for (int iu = 0; iu < nu; ++iu) {
+            const double u = u_first + iu * d.du;
+            BpViewU &W = viewu[(size_t)i * nu + iu];
+            const double Ax = (-d.sdd * c - u * s) / d.dx, Ay = (-d.sdd * s + u * c) / d.dy;
+            W.Ax = (float)Ax; W.Ay = (float)Ay;
+            W.Wx = (float)(1.0 / nudge(Ax, 1e-6 * d.sdd / d.dx)); W.Wy = (float)(1.0 / nudge(Ay, 1e-6 * d.sdd / d.dy));
+            W.Gx = (float)(-d.sad * u * s / d.dx); W.Gy = (float)(d.sad * u * c / d.dy);
+            W.pad0 = W.pad1 = 0.f;
+        }
+    }
+    for (int iv = 0; iv < nv; ++iv) {
+        const double v = v_first + iv * d.dv, vz = v / d.dz;
+        rows[iv] = make_float2((float)vz, (float)(1.0 / nudge(vz, 1e-6 * d.sdd / d.dz)));
+        for (int iu = 0; iu < nu; ++iu) {
+            const double u = u_first + iu * d.du;
+            const double L = std::sqrt(d.sdd * d.sdd + u * u + v * v);
+            const double q = (u * u + v * v) / (L * (L + d.sdd));                 // 1 - SDD/L without cancellation
+            pix[(size_t)iv * nu + iu] = make_float4((float)(1.0 / L), (float)q, (float)L, 0.f);
+        }
+    }
+    BpTables &T = G->bp;
+    const size_t ncell = (size_t)(d.nx + 1) * (d.ny + 1) * (d.nz + 1);
+    cudaError_t e = cudaMalloc((void **)&T.views, sizeof(BpView) * views.size());
+    if (e == cudaSuccess) e = cudaMalloc((void **)&T.viewu, sizeof(BpViewU) * viewu.size());
+    if (e == cudaSuccess) e = cudaMalloc((void **)&T.pix, sizeof(float4) * pix.size());
+    if (e == cudaSuccess) e = cudaMalloc((void **)&T.rows, sizeof(float2) * rows.size());
+    if (e == cudaSuccess) e = cudaMalloc((void **)&G->d_bp_partial, sizeof(float) * 8 * ncell);
+    if (e == cudaSuccess) e = cudaMemcpy((void *)T.views, views.data(), sizeof(BpView) * views.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy((void *)T.viewu, viewu.data(), sizeof(BpViewU) * viewu.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy((void *)T.pix, pix.data(), sizeof(float4) * pix.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy((void *)T.rows, rows.data(), sizeof(float2) * rows.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return set_cuda_error(e);
+    T.Kz = (float)cz0; T.cx0 = (float)cx0; T.cy0 = (float)cy0; T.cz0 = (float)cz0;
+    T.sdd = (float)d.sdd; T.sad = (float)d.sad; T.u_first = (float)u_first; T.inv_du = (float)(1.0 / d.du);
+    T.dz_dv = (float)(d.dz / d.dv); T.vfirst_dv = (float)(v_first / d.dv);
+    T.t0 = (float)(G->t_min + 0.5 * G->step); T.inv_step = (float)(1.0 / G->step);
+    T.k_eps = (float)std::fmax(0.02, 4.0 * 1.2e-7 * (d.sad + G->R) / G->step);   // fp32 rounding of r*L, in samples
+    T.stepf = (float)G->step; T.tau0f = (float)(G->t_min + 0.5 * G->step - d.sad);
+    G->workspace_bytes += sizeof(BpView) * views.size() + sizeof(BpViewU) * viewu.size() + sizeof(float4) * pix.size() +
+                          sizeof(float2) * rows.size() + sizeof(float) * 8 * ncell;
+    return CBCT_OK;
+}
+
 int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
     const DevGeom &g = G->dg;
     ProfScope prof(PROF_BACK, st);
-    dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4), g.nz);
-    backproject_gather_kernel<<<grid, block, 0, st>>>(g, d_proj, d_vol);
-    CBCT_LAUNCH_CHECK();
+    const char *impl = getenv("CBCT_BACKPROJECT_IMPL");              // "gather" forces the per-voxel kernel (tests)
+    if (impl && impl[0] == 'g') {
+        dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4), g.nz);
+        backproject_gather_kernel<<<grid, block, 0, st>>>(g, d_proj, d_vol);
+        CBCT_LAUNCH_CHECK();
+        return CBCT_OK;
+    }
+    {
+        dim3 block(32, 4), grid(cdiv(g.nx + 1, 32), cdiv(g.ny + 1, 4), g.nz + 1);
+        backproject_cell_kernel<<<grid, block, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K, d_proj,
+                                                         G->d_bp_partial);
+        CBCT_LAUNCH_CHECK();
+    }
+    {
+        dim3 block(32, 8), grid(cdiv(g.nx, 32), cdiv(g.ny, 8), g.nz);
+        backproject_combine_kernel<<<grid, block, 0, st>>>(G->d_bp_partial, d_vol, g.nx, g.ny, g.nz, (float)G->step);
+        CBCT_LAUNCH_CHECK();
+    }
     return CBCT_OK;
 }
 

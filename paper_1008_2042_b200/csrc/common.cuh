@@ -74,6 +74,32 @@ __device__ __forceinline__ void ray_setup(const DevGeom &g, int view, int iv, in
     r.bx = (float)bxd; r.by = (float)byd; r.bz = (float)bzd;
 }
 
+// ---- P^T (cell-driven) tables, built in fp64 at geometry create, stored fp32 ------------------------
+// With r = t / L(u,v) (t = distance from the source) a ray is  X = Kx + Ax r,  Y = Ky + Ay r,  Z = Kz + vz r,
+// so clipping against a cell is done in r and only then scaled by L.  Sample positions use the
+// re-anchored form  X = cX + bX * tau  (tau = t - SAD) with cX built from cancellation-free terms.
+struct BpView {                 // per view
+    float Kx, Ky;               // source position in index coordinates
+    float Fx, Fy;               // SAD cos/dx, SAD sin/dy
+    float D0, Dx, Dy;           // depth  D   = SAD - (x cos + y sin) as an affine function of cell indices (mm)
+    float T0, Tx, Ty;           // lateral tau = -x sin + y cos, same (mm)
+    float hl, hd;               // half lateral / half depth extent of one cell (mm)
+};
+struct BpViewU {                // per (view, iu)
+    float Ax, Ay;               // (-SDD cos - u sin)/dx, (-SDD sin + u cos)/dy
+    float Wx, Wy;               // 1/Ax, 1/Ay (denominators nudged away from 0; used for clipping only)
+    float Gx, Gy;               // -SAD u sin/dx, SAD u cos/dy
+    float pad0, pad1;
+};
+struct BpTables {
+    const BpView *views;        // [n_views]
+    const BpViewU *viewu;       // [n_views][nu]
+    const float4 *pix;          // [nv][nu]: {1/L, q = 1 - SDD/L, L, 0},  L = sqrt(SDD^2 + u^2 + v^2)
+    const float2 *rows;         // [nv]: {vz = v/dz, 1/vz (nudged)}
+    float Kz, cx0, cy0, cz0;    // Kz = cz0: index coordinate of the plane z = 0
+    float sdd, sad, u_first, inv_du, dz_dv, vfirst_dv, t0, inv_step, stepf, tau0f, k_eps;
+};
+
 }  // namespace cbct
 
 // ---- opaque handles --------------------------------------------------------------------------------
@@ -86,7 +112,8 @@ struct cbct_geometry {
     cbct::DevGeom dg;
     double2 *d_view_cs;
     float *d_ws_vol, *d_ws_proj;        // staging for the *_host entry points (allocated at create)
-    float *d_bp_partial;                // P^T workspace (per-corner partial volumes), may be null
+    float *d_bp_partial;                // P^T workspace: 8 per-corner partial volumes over the (n+1)^3 cells
+    cbct::BpTables bp;                  // P^T lookup tables (device pointers + constants)
     size_t workspace_bytes;
 };
 
@@ -103,6 +130,8 @@ namespace cbct {
 // kernels' host launchers used across translation units
 int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
 int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
+int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
+void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,
                  cudaStream_t st);
 constexpr int kReduceBlocks = 1184;     // 148 SMs x 8

@@ -165,6 +165,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
     G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr;
+    G->bp = BpTables{};
     G->workspace_bytes = 0;
 
     std::vector<double2> cs(desc->n_views);
@@ -190,6 +191,11 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     g.tau0 = G->t_min + 0.5 * step - desc->sad;
     g.view_cs = G->d_view_cs;
 
+    {
+        const int st_bp = build_bp_tables(G);
+        if (st_bp != CBCT_OK) { cbct_geometry_destroy(G); return st_bp; }
+    }
+
     // algorithmic sample count (unit of Gsamples/s), once, on the device
     const int blocks = 592;
     double *d_part = nullptr;
@@ -212,7 +218,7 @@ extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     cudaFree(G->d_view_cs);
     cudaFree(G->d_ws_vol);
     cudaFree(G->d_ws_proj);
-    cudaFree(G->d_bp_partial);
+    free_bp_tables(G);
     (void)cudaGetLastError();
     delete G;
     return CBCT_OK;
