@@ -95,17 +95,41 @@ __global__ void __launch_bounds__(128) backproject_gather_kernel(DevGeom g, cons
 //   per row: clip against the z slab, k-range of the global sample grid, then the samples.
 // A sample belongs to the cell iff floor(X,Y,Z) == (ix,iy,iz), evaluated on the same fp32 X,Y,Z in
 // every thread, so each sample is counted exactly once however the clipping rounds.
+// Lane mapping: the 32 lanes of a warp are cells that are neighbours ALONG Z (same ix, iy): they share
+// the column loop and the x,y clip exactly, and their row loops and sample counts have (nearly) equal
+// trip counts, so the warp stays converged.  Projections and the per-pixel table are read through
+// v-fastest (transposed) copies so that those lanes touch neighbouring addresses.
 // ------------------------------------------------------------------------------------------------
 constexpr float BP_EPS = 0.02f;
 
-__global__ void __launch_bounds__(128) backproject_cell_kernel(BpTables P, int nx, int ny, int nz, int nu, int nv,
-                                                               int n_views, int K, const float *__restrict__ proj,
+// gT[view][iu][iv] = g[view][iv][iu]
+__global__ void __launch_bounds__(256) transpose_proj_kernel(const float *__restrict__ g, float *__restrict__ gT, int nu,
+                                                             int nv) {
+    __shared__ float tile[32][33];
+    const size_t base = (size_t)blockIdx.z * nu * nv;
+    const int u0 = blockIdx.x * 32, v0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int u = u0 + threadIdx.x, v = v0 + j;
+        if (u < nu && v < nv) tile[j][threadIdx.x] = __ldg(g + base + (size_t)v * nu + u);
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int u = u0 + j, v = v0 + threadIdx.x;
+        if (u < nu && v < nv) gT[base + (size_t)u * nv + v] = tile[threadIdx.x][j];
+    }
+}
+
+__global__ void __launch_bounds__(512) backproject_cell_kernel(BpTables P, int nx, int ny, int nz, int nu, int nv,
+                                                               int n_views, int K, int xb, const float *__restrict__ projT,
                                                                float *__restrict__ partial) {
-    const int ix = blockIdx.x * 32 + threadIdx.x - 1, iy = blockIdx.y * 4 + threadIdx.y - 1, iz = blockIdx.z - 1;
-    if (ix > nx - 1 || iy > ny - 1) return;
+    const int nzc = nz + 1;
+    const int xr = (int)threadIdx.x / nzc, zc = (int)threadIdx.x - xr * nzc;
+    const int ix = blockIdx.x * xb + xr - 1, iy = (int)blockIdx.y - 1, iz = zc - 1;
+    if (xr >= xb || ix > nx - 1) return;
     const float fix = (float)ix, fiy = (float)iy, fiz = (float)iz;
     const float az = fiz - P.Kz, bz = az + 1.f;
     float a000 = 0.f, a100 = 0.f, a010 = 0.f, a110 = 0.f, a001 = 0.f, a101 = 0.f, a011 = 0.f, a111 = 0.f;
+    const float k_off = -(P.t0 * P.inv_step);
     for (int view = 0; view < n_views; ++view) {
         const BpView V = P.views[view];
         // candidate columns: projected cell centre +- conservative half width
@@ -116,8 +140,8 @@ __global__ void __launch_bounds__(128) backproject_cell_kernel(BpTables P, int n
         const float dumax = P.sdd * rDn * fmaf(fabsf(tc) * rD, V.hd, V.hl);
         const int iu0 = max(0, (int)ceilf((uc - dumax - P.u_first) * P.inv_du - BP_EPS));
         const int iu1 = min(nu - 1, (int)floorf((uc + dumax - P.u_first) * P.inv_du + BP_EPS));
-        const BpViewU *vu = P.viewu + (size_t)view * nu;
-        const float *pv = proj + (size_t)view * nv * nu;
+        const BpViewU *vu = P.viewu + view * nu;
+        const float *pv = projT + (size_t)view * nv * nu;
         for (int iu = iu0; iu <= iu1; ++iu) {
             const float4 w0 = __ldg(reinterpret_cast<const float4 *>(vu + iu));        // Ax Ay Wx Wy
             const float rx0 = (fix - V.Kx) * w0.z, rx1 = rx0 + w0.z;
@@ -129,25 +153,31 @@ __global__ void __launch_bounds__(128) backproject_cell_kernel(BpTables P, int n
             const float vzmin = fminf(az * i_in, az * i_out), vzmax = fmaxf(bz * i_in, bz * i_out);
             const int iv0 = max(0, (int)ceilf(fmaf(vzmin, P.dz_dv, -P.vfirst_dv) - BP_EPS));
             const int iv1 = min(nv - 1, (int)floorf(fmaf(vzmax, P.dz_dv, -P.vfirst_dv) + BP_EPS));
+            const float4 *pp = P.pixT + iu * nv;
+            const float *gp = pv + iu * nv;
             for (int iv = iv0; iv <= iv1; ++iv) {
                 const float2 rw = __ldg(P.rows + iv);                                  // vz, 1/vz
                 const float rz0 = az * rw.y, rz1 = bz * rw.y;
                 const float rlo = fmaxf(rin, fminf(rz0, rz1)), rhi = fminf(rout, fmaxf(rz0, rz1));
                 if (!(rlo <= rhi)) continue;
-                const float4 t = __ldg(P.pix + (size_t)iv * nu + iu);                  // 1/L, q, L
-                const int ka = max(0, (int)ceilf(fmaf(rlo, t.z, -P.t0) * P.inv_step - P.k_eps));
-                const int kb = min(K - 1, (int)floorf(fmaf(rhi, t.z, -P.t0) * P.inv_step + P.k_eps));
+                const float4 t = __ldg(pp + iv);                                       // 1/L, q, L
+                const float sl = t.z * P.inv_step;
+                const int ka = max(0, (int)ceilf(fmaf(rlo, sl, k_off) - P.k_eps));
+                const int kb = min(K - 1, (int)floorf(fmaf(rhi, sl, k_off) + P.k_eps));
                 if (ka > kb) continue;
-                const float gval = __ldg(pv + (size_t)iv * nu + iu);
+                const float gval = __ldg(gp + iv);
                 const float bx = w0.x * t.x, by = w0.y * t.x, bzz = rw.x * t.x;
                 const float cx = fmaf(w1.x, t.x, fmaf(V.Fx, t.y, P.cx0));
                 const float cy = fmaf(w1.y, t.x, fmaf(V.Fy, t.y, P.cy0));
                 const float cz = fmaf(P.sad * rw.x, t.x, P.cz0);
-                for (int k = ka; k <= kb; ++k) {
-                    const float tau = fmaf((float)k, P.stepf, P.tau0f);
+                float kf = (float)ka;
+                for (int k = ka; k <= kb; ++k, kf += 1.f) {
+                    const float tau = fmaf(kf, P.stepf, P.tau0f);
                     // X,Y,Z depend on (view, iu, iv, k) only, so all cells agree on them; X - ix is exact
                     const float fx = fmaf(bx, tau, cx) - fix, fy = fmaf(by, tau, cy) - fiy, fz = fmaf(bzz, tau, cz) - fiz;
-                    const bool in = fx >= 0.f && fx < 1.f && fy >= 0.f && fy < 1.f && fz >= 0.f && fz < 1.f;
+                    // 0 <= f < 1 on all three axes, as one unsigned compare each (negative floats have the sign bit set)
+                    const bool in = __float_as_uint(fx) < 0x3f800000u && __float_as_uint(fy) < 0x3f800000u &&
+                                    __float_as_uint(fz) < 0x3f800000u;
                     const float gg = in ? gval : 0.f;
                     const float g1 = gg * fz, g0 = gg - g1;
                     const float g01 = g0 * fy, g00 = g0 - g01, g11 = g1 * fy, g10 = g1 - g11;
@@ -160,33 +190,46 @@ __global__ void __launch_bounds__(128) backproject_cell_kernel(BpTables P, int n
             }
         }
     }
-    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * (nz + 1);
-    const size_t ci = ((size_t)(iz + 1) * (ny + 1) + (iy + 1)) * (nx + 1) + (ix + 1);
+    // partial[corner][(iy+1)][(ix+1)][(iz+1)], z fastest: lanes write neighbouring words
+    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * nzc;
+    const size_t ci = ((size_t)(iy + 1) * (nx + 1) + (ix + 1)) * nzc + zc;
     partial[ci] = a000; partial[ncell + ci] = a100; partial[2 * ncell + ci] = a010; partial[3 * ncell + ci] = a110;
     partial[4 * ncell + ci] = a001; partial[5 * ncell + ci] = a101; partial[6 * ncell + ci] = a011;
     partial[7 * ncell + ci] = a111;
 }
 
-// voxel (x,y,z) = step * sum over the 8 cells (x-dx, y-dy, z-dz) of their corner (dx,dy,dz) accumulator
-__global__ void __launch_bounds__(256) backproject_combine_kernel(const float *__restrict__ partial, float *__restrict__ vol,
+// voxel (x,y,z) = step * sum over the 8 cells (x-dx, y-dy, z-dz) of their corner (dx,dy,dz) accumulator.
+// One thread per (x,y) column walking z: lanes are neighbours in x (coalesced float stores), and the
+// z-fastest partials are re-used from L1 along the walk.
+__global__ void __launch_bounds__(128) backproject_combine_kernel(const float *__restrict__ partial, float *__restrict__ vol,
                                                                   int nx, int ny, int nz, float stepf) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y * blockDim.y + threadIdx.y, z = blockIdx.z;
+    const int x = blockIdx.x * 32 + threadIdx.x, y = blockIdx.y * 4 + threadIdx.y;
     if (x >= nx || y >= ny) return;
-    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * (nz + 1);
-    float acc = 0.f;
+    const int nzc = nz + 1;
+    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * nzc;
+    const float *col[4];
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        const int dx = c & 1, dy = (c >> 1) & 1, dz = c >> 2;
-        const size_t ci = ((size_t)(z - dz + 1) * (ny + 1) + (y - dy + 1)) * (nx + 1) + (x - dx + 1);
-        acc += __ldg(partial + (size_t)c * ncell + ci);
+    for (int c = 0; c < 4; ++c) {
+        const int dx = c & 1, dy = c >> 1;
+        col[c] = partial + ((size_t)(y - dy + 1) * (nx + 1) + (x - dx + 1)) * nzc + (size_t)c * ncell;
     }
-    vol[((size_t)z * ny + y) * nx + x] = acc * stepf;
+    for (int z = 0; z < nz; ++z) {
+        float acc = 0.f;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int dz = c >> 2;
+            acc += __ldg(col[c & 3] + (size_t)dz * 4 * ncell + (z - dz + 1));
+        }
+        vol[((size_t)z * ny + y) * nx + x] = acc * stepf;
+    }
 }
 
 void free_bp_tables(cbct_geometry *G) {
     cudaFree(const_cast<BpView *>(G->bp.views));
     cudaFree(const_cast<BpViewU *>(G->bp.viewu));
-    cudaFree(const_cast<float4 *>(G->bp.pix));
+    cudaFree(const_cast<float4 *>(G->bp.pixT));
+    cudaFree(G->d_bp_projT);
+    G->d_bp_projT = nullptr;
     cudaFree(const_cast<float2 *>(G->bp.rows));
     cudaFree(G->d_bp_partial);
     G->bp = BpTables{};
@@ -203,7 +246,7 @@ int build_bp_tables(cbct_geometry *G) {
     const int nu = d.nu, nv = d.nv, nvw = d.n_views;
     std::vector<BpView> views(nvw);
     std::vector<BpViewU> viewu((size_t)nvw * nu);
-    std::vector<float4> pix((size_t)nv * nu);
+    std::vector<float4> pix((size_t)nv * nu);   // stored v-fastest: pixT[iu][iv]
     std::vector<float2> rows(nv);
     const double cx0 = -d.ox / d.dx + 0.5 * (d.nx - 1), cy0 = -d.oy / d.dy + 0.5 * (d.ny - 1),
                  cz0 = -d.oz / d.dz + 0.5 * (d.nz - 1);
@@ -237,19 +280,20 @@ int build_bp_tables(cbct_geometry *G) {
             const double u = u_first + iu * d.du;
             const double L = std::sqrt(d.sdd * d.sdd + u * u + v * v);
             const double q = (u * u + v * v) / (L * (L + d.sdd));                 // 1 - SDD/L without cancellation
-            pix[(size_t)iv * nu + iu] = make_float4((float)(1.0 / L), (float)q, (float)L, 0.f);
+            pix[(size_t)iu * nv + iv] = make_float4((float)(1.0 / L), (float)q, (float)L, 0.f);
         }
     }
     BpTables &T = G->bp;
     const size_t ncell = (size_t)(d.nx + 1) * (d.ny + 1) * (d.nz + 1);
     cudaError_t e = cudaMalloc((void **)&T.views, sizeof(BpView) * views.size());
     if (e == cudaSuccess) e = cudaMalloc((void **)&T.viewu, sizeof(BpViewU) * viewu.size());
-    if (e == cudaSuccess) e = cudaMalloc((void **)&T.pix, sizeof(float4) * pix.size());
+    if (e == cudaSuccess) e = cudaMalloc((void **)&T.pixT, sizeof(float4) * pix.size());
     if (e == cudaSuccess) e = cudaMalloc((void **)&T.rows, sizeof(float2) * rows.size());
     if (e == cudaSuccess) e = cudaMalloc((void **)&G->d_bp_partial, sizeof(float) * 8 * ncell);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&G->d_bp_projT, sizeof(float) * G->n_rays);
     if (e == cudaSuccess) e = cudaMemcpy((void *)T.views, views.data(), sizeof(BpView) * views.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy((void *)T.viewu, viewu.data(), sizeof(BpViewU) * viewu.size(), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy((void *)T.pix, pix.data(), sizeof(float4) * pix.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy((void *)T.pixT, pix.data(), sizeof(float4) * pix.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy((void *)T.rows, rows.data(), sizeof(float2) * rows.size(), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return set_cuda_error(e);
     T.Kz = (float)cz0; T.cx0 = (float)cx0; T.cy0 = (float)cy0; T.cz0 = (float)cz0;
@@ -259,7 +303,7 @@ int build_bp_tables(cbct_geometry *G) {
     T.k_eps = (float)std::fmax(0.02, 4.0 * 1.2e-7 * (d.sad + G->R) / G->step);   // fp32 rounding of r*L, in samples
     T.stepf = (float)G->step; T.tau0f = (float)(G->t_min + 0.5 * G->step - d.sad);
     G->workspace_bytes += sizeof(BpView) * views.size() + sizeof(BpViewU) * viewu.size() + sizeof(float4) * pix.size() +
-                          sizeof(float2) * rows.size() + sizeof(float) * 8 * ncell;
+                          sizeof(float2) * rows.size() + sizeof(float) * 8 * ncell + sizeof(float) * G->n_rays;
     return CBCT_OK;
 }
 
@@ -274,13 +318,27 @@ int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol
         return CBCT_OK;
     }
     {
-        dim3 block(32, 4), grid(cdiv(g.nx + 1, 32), cdiv(g.ny + 1, 4), g.nz + 1);
-        backproject_cell_kernel<<<grid, block, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K, d_proj,
-                                                         G->d_bp_partial);
+        dim3 block(32, 8), grid(cdiv(g.nu, 32), cdiv(g.nv, 32), g.n_views);
+        transpose_proj_kernel<<<grid, block, 0, st>>>(d_proj, G->d_bp_projT, g.nu, g.nv);
         CBCT_LAUNCH_CHECK();
     }
     {
-        dim3 block(32, 8), grid(cdiv(g.nx, 32), cdiv(g.ny, 8), g.nz);
+        // block = xb x-neighbouring columns of nz+1 cells, lanes along z; xb minimises idle lanes
+        const int nzc = g.nz + 1;
+        int xb = 1, best_waste = 1 << 30;
+        for (int c = 1; c <= 16 && c * nzc <= 512; ++c) {
+            const int th = ((c * nzc + 31) / 32) * 32, waste = (th - c * nzc) * 1024 / th;
+            if (th >= 128 && waste < best_waste) { best_waste = waste; xb = c; }
+        }
+        if (nzc > 512) return CBCT_E_UNSUPPORTED;   // taller volumes: use CBCT_BACKPROJECT_IMPL=gather
+        const int threads = ((xb * nzc + 31) / 32) * 32;
+        dim3 grid(cdiv(g.nx + 1, xb), g.ny + 1);
+        backproject_cell_kernel<<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K, xb,
+                                                           G->d_bp_projT, G->d_bp_partial);
+        CBCT_LAUNCH_CHECK();
+    }
+    {
+        dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4));
         backproject_combine_kernel<<<grid, block, 0, st>>>(G->d_bp_partial, d_vol, g.nx, g.ny, g.nz, (float)G->step);
         CBCT_LAUNCH_CHECK();
     }

@@ -94,7 +94,7 @@ struct BpViewU {                // per (view, iu)
 struct BpTables {
     const BpView *views;        // [n_views]
     const BpViewU *viewu;       // [n_views][nu]
-    const float4 *pix;          // [nv][nu]: {1/L, q = 1 - SDD/L, L, 0},  L = sqrt(SDD^2 + u^2 + v^2)
+    const float4 *pixT;         // [nu][nv] (v fastest): {1/L, q = 1 - SDD/L, L, 0},  L = sqrt(SDD^2 + u^2 + v^2)
     const float2 *rows;         // [nv]: {vz = v/dz, 1/vz (nudged)}
     float Kz, cx0, cy0, cz0;    // Kz = cz0: index coordinate of the plane z = 0
     float sdd, sad, u_first, inv_du, dz_dv, vfirst_dv, t0, inv_step, stepf, tau0f, k_eps;
@@ -113,6 +113,7 @@ struct cbct_geometry {
     double2 *d_view_cs;
     float *d_ws_vol, *d_ws_proj;        // staging for the *_host entry points (allocated at create)
     float *d_bp_partial;                // P^T workspace: 8 per-corner partial volumes over the (n+1)^3 cells
+    float *d_bp_projT;                  // P^T workspace: projections transposed to [view][iu][iv]
     cbct::BpTables bp;                  // P^T lookup tables (device pointers + constants)
     size_t workspace_bytes;
 };

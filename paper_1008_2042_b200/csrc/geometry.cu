@@ -164,7 +164,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     G->K = (int32_t)std::ceil(2.0 * R / step);
     G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
-    G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr;
+    G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr;
     G->bp = BpTables{};
     G->workspace_bytes = 0;
 
