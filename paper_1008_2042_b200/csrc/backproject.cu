@@ -4,6 +4,7 @@
 //   f_j = step * sum_rays g_ray * sum_k hat(X_k - jx) hat(Y_k - jy) hat(Z_k - jz)
 // (SURVEY.md §8(c) c.3).  No atomics: each output voxel is owned by one thread, so the result is
 // deterministic.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <vector>
@@ -119,7 +120,8 @@ __global__ void __launch_bounds__(256) transpose_proj_kernel(const float *__rest
     }
 }
 
-__global__ void __launch_bounds__(512) backproject_cell_kernel(BpTables P, int nx, int ny, int nz, int nu, int nv,
+template <int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) backproject_cell_kernel(BpTables P, int nx, int ny, int nz, int nu, int nv,
                                                                int n_views, int K, int xb, const float *__restrict__ projT,
                                                                float *__restrict__ partial) {
     const int nzc = nz + 1;
@@ -129,7 +131,8 @@ __global__ void __launch_bounds__(512) backproject_cell_kernel(BpTables P, int n
     const float fix = (float)ix, fiy = (float)iy, fiz = (float)iz;
     const float az = fiz - P.Kz, bz = az + 1.f;
     float a000 = 0.f, a100 = 0.f, a010 = 0.f, a110 = 0.f, a001 = 0.f, a101 = 0.f, a011 = 0.f, a111 = 0.f;
-    const float k_off = -(P.t0 * P.inv_step);
+    const float inv_step = P.inv_step, stepf = P.stepf, tau0f = P.tau0f;
+    const float k_lo_off = -(P.t0 * P.inv_step) - P.k_eps, k_hi_off = -(P.t0 * P.inv_step) + P.k_eps;
     for (int view = 0; view < n_views; ++view) {
         const BpView V = P.views[view];
         // candidate columns: projected cell centre +- conservative half width
@@ -153,26 +156,27 @@ __global__ void __launch_bounds__(512) backproject_cell_kernel(BpTables P, int n
             const float vzmin = fminf(az * i_in, az * i_out), vzmax = fmaxf(bz * i_in, bz * i_out);
             const int iv0 = max(0, (int)ceilf(fmaf(vzmin, P.dz_dv, -P.vfirst_dv) - BP_EPS));
             const int iv1 = min(nv - 1, (int)floorf(fmaf(vzmax, P.dz_dv, -P.vfirst_dv) + BP_EPS));
-            const float4 *pp = P.pixT + iu * nv;
-            const float *gp = pv + iu * nv;
-            for (int iv = iv0; iv <= iv1; ++iv) {
-                const float2 rw = __ldg(P.rows + iv);                                  // vz, 1/vz
+            // running pointers (v-fastest tables): one add per row instead of 64-bit index arithmetic
+            const float4 *pp = P.pixT + (iu * nv + iv0);
+            const float *gp = pv + (iu * nv + iv0);
+            const float2 *rp = P.rows + iv0;
+            for (int iv = iv0; iv <= iv1; ++iv, ++pp, ++gp, ++rp) {
+                const float2 rw = __ldg(rp);                                           // vz, 1/vz
+                const float4 t = __ldg(pp);                                            // 1/L, q, L
+                const float gval = __ldg(gp);                                          // all three loads in flight together
                 const float rz0 = az * rw.y, rz1 = bz * rw.y;
                 const float rlo = fmaxf(rin, fminf(rz0, rz1)), rhi = fminf(rout, fmaxf(rz0, rz1));
-                if (!(rlo <= rhi)) continue;
-                const float4 t = __ldg(pp + iv);                                       // 1/L, q, L
-                const float sl = t.z * P.inv_step;
-                const int ka = max(0, (int)ceilf(fmaf(rlo, sl, k_off) - P.k_eps));
-                const int kb = min(K - 1, (int)floorf(fmaf(rhi, sl, k_off) + P.k_eps));
-                if (ka > kb) continue;
-                const float gval = __ldg(gp + iv);
+                const float sl = t.z * inv_step;
+                const int ka = max(0, (int)ceilf(fmaf(rlo, sl, k_lo_off)));
+                const int kb = min(K - 1, (int)floorf(fmaf(rhi, sl, k_hi_off)));
+                if (ka > kb) continue;                                                 // also rejects rlo > rhi
                 const float bx = w0.x * t.x, by = w0.y * t.x, bzz = rw.x * t.x;
                 const float cx = fmaf(w1.x, t.x, fmaf(V.Fx, t.y, P.cx0));
                 const float cy = fmaf(w1.y, t.x, fmaf(V.Fy, t.y, P.cy0));
                 const float cz = fmaf(P.sad * rw.x, t.x, P.cz0);
                 float kf = (float)ka;
                 for (int k = ka; k <= kb; ++k, kf += 1.f) {
-                    const float tau = fmaf(kf, P.stepf, P.tau0f);
+                    const float tau = fmaf(kf, stepf, tau0f);
                     // X,Y,Z depend on (view, iu, iv, k) only, so all cells agree on them; X - ix is exact
                     const float fx = fmaf(bx, tau, cx) - fix, fy = fmaf(by, tau, cy) - fiy, fz = fmaf(bzz, tau, cz) - fiz;
                     // 0 <= f < 1 on all three axes, as one unsigned compare each (negative floats have the sign bit set)
@@ -326,15 +330,23 @@ int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol
         // block = xb x-neighbouring columns of nz+1 cells, lanes along z; xb minimises idle lanes
         const int nzc = g.nz + 1;
         int xb = 1, best_waste = 1 << 30;
-        for (int c = 1; c <= 16 && c * nzc <= 512; ++c) {
+        const char *mt = getenv("CBCT_BP_MAXT");
+        const int max_threads = mt ? atoi(mt) : 320;
+        for (int c = 1; c <= 16 && c * nzc <= max_threads; ++c) {
             const int th = ((c * nzc + 31) / 32) * 32, waste = (th - c * nzc) * 1024 / th;
             if (th >= 128 && waste < best_waste) { best_waste = waste; xb = c; }
         }
+        if (best_waste == (1 << 30)) xb = nzc <= 512 ? std::max(1, std::min(16, 512 / nzc)) : 1;
         if (nzc > 512) return CBCT_E_UNSUPPORTED;   // taller volumes: use CBCT_BACKPROJECT_IMPL=gather
         const int threads = ((xb * nzc + 31) / 32) * 32;
         dim3 grid(cdiv(g.nx + 1, xb), g.ny + 1);
-        backproject_cell_kernel<<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K, xb,
-                                                           G->d_bp_projT, G->d_bp_partial);
+        const char *var = getenv("CBCT_BP_VARIANT");                  // "4": 48-register build, 4 CTAs/SM (experiments)
+        if (threads <= 320 && var && var[0] == '4')
+            backproject_cell_kernel<320, 4><<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K,
+                                                                       xb, G->d_bp_projT, G->d_bp_partial);
+        else
+            backproject_cell_kernel<512, 2><<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K,
+                                                                       xb, G->d_bp_projT, G->d_bp_partial);
         CBCT_LAUNCH_CHECK();
     }
     {
