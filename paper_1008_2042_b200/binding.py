@@ -189,7 +189,11 @@ class Geometry:
             lib().cbct_geometry_destroy(self.handle)
             self.handle = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:      # interpreter shutdown: module globals may already be gone
+            pass
 
     def forward(self, d_vol, d_proj, stream=None):
         _check(lib().cbct_forward(self.handle, _dptr(d_vol, self.n_vox), _dptr(d_proj, self.n_rays), _stream(stream)),
@@ -226,7 +230,11 @@ class Cgls:
             lib().cbct_cgls_destroy(self.handle)
             self.handle = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:      # interpreter shutdown: module globals may already be gone
+            pass
 
     def init(self, d_g, d_x, d_r, d_p, stream=None):
         G = self.geometry
@@ -314,7 +322,11 @@ class Recon:
             lib().cbct_recon_destroy(self.handle)
             self.handle = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:      # interpreter shutdown: module globals may already be gone
+            pass
 
     def _outer(self, n_outer: Sequence[int]):
         assert len(n_outer) == self.n_levels

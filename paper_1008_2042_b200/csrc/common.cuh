@@ -115,6 +115,11 @@ struct cbct_geometry {
     float *d_bp_partial;                // P^T workspace: 8 per-corner partial volumes over the (n+1)^3 cells
     float *d_bp_projT;                  // P^T workspace: projections transposed to [view][iu][iv]
     cbct::BpTables bp;                  // P^T lookup tables (device pointers + constants)
+    // forward TMA path (forward_tma.cu): box plan, y-fastest volume copy and its tensor map
+    int fw_tma_ok, fw_b, fw_bz;
+    float fw_margin;
+    float *d_fw_volT;
+    alignas(64) unsigned char fw_map_y[128];
     size_t workspace_bytes;
 };
 
@@ -131,6 +136,8 @@ namespace cbct {
 // kernels' host launchers used across translation units
 int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
 int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
+void plan_forward_tma(cbct_geometry *g);     // decides whether/how the TMA forward kernel runs for this geometry
+int launch_forward_tma(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
 int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
 void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,

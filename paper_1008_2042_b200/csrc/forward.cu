@@ -237,8 +237,9 @@ int launch_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, cu
     ProfScope prof(PROF_FORWARD, st);
     dim3 block(FW_TU, FW_TV), grid(cdiv(g.nu, FW_TU), cdiv(g.nv, FW_TV), g.n_views);
     float margin = 0.f;
-    const char *impl = getenv("CBCT_FORWARD_IMPL");                  // "global" forces the untiled kernel (tests)
-    const bool want_global = impl && impl[0] == 'g';
+    const char *impl = getenv("CBCT_FORWARD_IMPL");                  // "global" / "tiled" force the older kernels (tests)
+    const bool want_global = impl && impl[0] == 'g', want_tiled = impl && impl[0] == 't' && impl[1] == 'i';
+    if (!want_global && !want_tiled && launch_forward_tma(G, d_vol, d_proj, st) == CBCT_OK) return CBCT_OK;
     if (!want_global && tiled_fits(G, &margin))
         forward_tiled_kernel<<<grid, block, 0, st>>>(g, d_vol, d_proj, margin);
     else

@@ -1,0 +1,361 @@
+// forward_tma.cu -- g = P f, the sm_100a fast path of cbct_forward (include/cbct.h).
+// Same arithmetic as forward.cu (Eq. 1 as a fixed-step sum of zero-padded trilinear
+// samples); what changes is how the volume reaches the SM:
+//   * a CTA owns a 16(u) x 16(v) pixel tile of one view and marches the global t-grid in chunks;
+//   * for every chunk ONE thread issues a TMA tensor copy (cp.async.bulk.tensor.3d) of the fixed-size
+//     voxel box that covers the tile's frustum segment; out-of-range coordinates are zero-filled by the
+//     TMA unit, which IS the zero padding of T.  Two boxes are in flight (mbarrier double buffering),
+//     so staging costs no instructions and overlaps the sampling of the previous chunk;
+//   * views whose detector u-axis is closer to y than to x read a y-fastest copy of the volume
+//     (transposed once per call), so that the 16 pixels of a half-warp always fall on neighbouring
+//     words of the fastest shared-memory axis (bank-conflict free for every view direction);
+//   * floor/fraction use the add-magic-number trick in round-down mode (no conversion instructions)
+//     and positions are kept relative to the box origin.
+#include <cuda.h>
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+#include "common.cuh"
+
+namespace cbct {
+
+constexpr int FT_TU = 16, FT_TV = 16, FT_THREADS = 256, FT_KCMAX = 64;
+constexpr float FT_MAGIC = 8388608.0f;          // 2^23: x + 2^23 rounded down has floor(x) in its low mantissa bits
+constexpr unsigned FT_MAGIC_BITS = 0x4B000000u;
+
+struct RayL { float cf, cs, cz, bf, bs, bz; };  // ray in (fast, slow, z) index coordinates: P(tau) = c + b tau
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+        : "memory");
+}
+
+struct Box3 { int lf, ls, lz; bool fits; };
+
+// origin of the box for samples tau_a..tau_b of the tile (AABB of the 4 corner rays at both ends grown by
+// `margin`), and whether its extents (+1 for the upper neighbour) fit the fixed box (bfs x bfs x bzz)
+__device__ __forceinline__ Box3 chunk_box(const RayL *corner, float tau_a, float tau_b, float margin, int bfs, int bzz) {
+    float mnf = 1e30f, mns = 1e30f, mnz = 1e30f, mxf = -1e30f, mxs = -1e30f, mxz = -1e30f;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const RayL r = corner[c];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const float tau = e ? tau_b : tau_a;
+            const float F = fmaf(r.bf, tau, r.cf), S = fmaf(r.bs, tau, r.cs), Z = fmaf(r.bz, tau, r.cz);
+            mnf = fminf(mnf, F); mxf = fmaxf(mxf, F);
+            mns = fminf(mns, S); mxs = fmaxf(mxs, S);
+            mnz = fminf(mnz, Z); mxz = fmaxf(mxz, Z);
+        }
+    }
+    Box3 b;
+    // TMA: the innermost start coordinate must keep the global address 16-byte aligned -> multiple of 4
+    b.lf = ((int)floorf(mnf - margin)) & ~3; b.ls = (int)floorf(mns - margin); b.lz = (int)floorf(mnz - margin);
+    const int hf = (int)floorf(mxf + margin) + 1, hs = (int)floorf(mxs + margin) + 1, hz = (int)floorf(mxz + margin) + 1;
+    b.fits = (hf - b.lf + 1 <= bfs) && (hs - b.ls + 1 <= bfs) && (hz - b.lz + 1 <= bzz);
+    return b;
+}
+
+struct ChunkPlan { int kc; Box3 box; float tau_base; };
+
+__device__ __forceinline__ ChunkPlan plan_chunk(const DevGeom &g, const RayL *corner, int k0, int K1, float margin, int bfs,
+                                                int bzz) {
+    ChunkPlan p;
+    p.tau_base = (float)(g.tau0 + (double)k0 * g.step);
+    const float stepf = (float)g.step;
+    int kc = min(FT_KCMAX, K1 - k0 + 1);
+    for (;;) {
+        p.box = chunk_box(corner, p.tau_base, fmaf((float)(kc - 1), stepf, p.tau_base), margin, bfs, bzz);
+        if (p.box.fits || kc == 1) break;
+        kc = (kc > 8) ? (kc * 3) >> 2 : kc - 1;            // 64, 48, 36, 27, 20, 15, 11, 8, 7, ...
+    }
+    p.kc = kc;
+    return p;
+}
+
+__device__ __forceinline__ float fetch0g(const float *__restrict__ vol, const DevGeom &g, int ix, int iy, int iz) {
+    if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) return 0.f;
+    return __ldg(vol + ((size_t)iz * g.ny + iy) * g.nx + ix);
+}
+
+__global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
+                                                                 const __grid_constant__ CUtensorMap map_y,
+                                                                 const float *__restrict__ vol, float *__restrict__ proj,
+                                                                 float margin, int bfs, int bzz, int dbg) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) unsigned long long bars[2];
+    __shared__ RayL corner[4];
+    __shared__ int s_klo, s_khi;
+    float *buf0 = reinterpret_cast<float *>(smem_raw);
+    const int box_elems = (bfs * bfs * bzz + 31) & ~31;   // buffer stride: keeps the second buffer 128-byte aligned
+    const unsigned box_bytes = (unsigned)(bfs * bfs * bzz) * 4u;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tu = lane & 15, tv = 2 * warp + (lane >> 4);
+    const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = blockIdx.z;
+    const bool valid = iu < g.nu && iv < g.nv;
+
+    // orientation: the detector u-axis is e_u = (-sin, cos); the fast shared-memory axis follows it
+    const double2 cs = g.view_cs[view];
+    const bool yfast = fabs(cs.x) > fabs(cs.y);
+
+    RayF r;
+    double b[3], c[3];
+    ray_setup(g, view, iv, iu, r, b[0], b[1], b[2], c[0], c[1], c[2]);
+    int klo = 0x7fffffff, khi = -1;
+    if (valid) {
+        const double hi[3] = {(double)g.nx, (double)g.ny, (double)g.nz};
+        double tin = -1e300, tout = 1e300;
+        bool miss = false;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (b[a] == 0.0) { miss |= (c[a] <= -1.0 || c[a] >= hi[a]); continue; }
+            const double inv = 1.0 / b[a];
+            double t1 = (-1.0 - c[a]) * inv, t2 = (hi[a] - c[a]) * inv;
+            if (t1 > t2) { const double t = t1; t1 = t2; t2 = t; }
+            tin = fmax(tin, t1); tout = fmin(tout, t2);
+        }
+        if (!miss && tout > tin) {
+            const long long a = (long long)ceil((tin - g.tau0) / g.step), e = (long long)floor((tout - g.tau0) / g.step);
+            klo = (int)max(a, 0LL); khi = (int)min(e, (long long)g.K - 1);
+            if (khi < klo) { klo = 0x7fffffff; khi = -1; }
+        }
+    }
+    RayL rl;
+    rl.cf = yfast ? r.cy : r.cx; rl.cs = yfast ? r.cx : r.cy; rl.cz = r.cz;
+    rl.bf = yfast ? r.by : r.bx; rl.bs = yfast ? r.bx : r.by; rl.bz = r.bz;
+
+    if (tid == 0) {
+        s_klo = 0x7fffffff; s_khi = -1;
+        mbar_init(smem_u32(&bars[0]), 1); mbar_init(smem_u32(&bars[1]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if ((tu == 0 || tu == FT_TU - 1) && (tv == 0 || tv == FT_TV - 1)) corner[(tv ? 2 : 0) + (tu ? 1 : 0)] = rl;
+    __syncthreads();
+    {
+        const int wlo = __reduce_min_sync(0xffffffffu, klo), whi = __reduce_max_sync(0xffffffffu, khi);
+        if (lane == 0) { atomicMin(&s_klo, wlo); atomicMax(&s_khi, whi); }
+    }
+    __syncthreads();
+    const int K0 = s_klo, K1 = s_khi;
+    const float stepf = (float)g.step;
+    const float sF = rl.bf * stepf, sS = rl.bs * stepf, sZ = rl.bz * stepf;
+    const int pS = bfs, pZ = bfs * bfs;
+    float total = 0.f;
+
+    if (K0 <= K1) {
+        ChunkPlan cur = plan_chunk(g, corner, K0, K1, margin, bfs, bzz);
+        if (tid == 0 && cur.box.fits && !(dbg & 1)) {
+            mbar_expect_tx(smem_u32(&bars[0]), box_bytes);
+            if (yfast) tma_load_3d(smem_u32(buf0), &map_y, cur.box.lf, cur.box.ls, cur.box.lz, smem_u32(&bars[0]));
+            else tma_load_3d(smem_u32(buf0), &map_x, cur.box.lf, cur.box.ls, cur.box.lz, smem_u32(&bars[0]));
+        }
+        unsigned phase0 = 0, phase1 = 0;
+        int k0 = K0, stage = 0;
+        while (k0 <= K1) {
+            const int kn = k0 + cur.kc;
+            ChunkPlan nxt = cur;
+            if (kn <= K1) {
+                nxt = plan_chunk(g, corner, kn, K1, margin, bfs, bzz);
+                if (tid == 0 && nxt.box.fits && !(dbg & 1)) {          // the other buffer was released by the barrier below
+                    const unsigned bar = smem_u32(&bars[stage ^ 1]);
+                    mbar_expect_tx(bar, box_bytes);
+                    const unsigned dst = smem_u32(buf0 + (stage ^ 1) * box_elems);
+                    if (yfast) tma_load_3d(dst, &map_y, nxt.box.lf, nxt.box.ls, nxt.box.lz, bar);
+                    else tma_load_3d(dst, &map_x, nxt.box.lf, nxt.box.ls, nxt.box.lz, bar);
+                }
+            }
+            const int ja = max(k0, klo), jb = min(kn - 1, khi);
+            if (cur.box.fits) {
+                if (!(dbg & 1)) mbar_wait(smem_u32(&bars[stage]), stage ? phase1 : phase0);
+                if (stage) phase1 ^= 1; else phase0 ^= 1;
+                if (ja <= jb && !(dbg & 2)) {
+                    // local coordinates: sample j sits at F0 + (j - ja) * sF, etc.
+                    const float tau_a = fmaf((float)(ja - k0), stepf, cur.tau_base);
+                    const float F0 = fmaf(rl.bf, tau_a, rl.cf - (float)cur.box.lf);
+                    const float S0 = fmaf(rl.bs, tau_a, rl.cs - (float)cur.box.ls);
+                    const float Z0 = fmaf(rl.bz, tau_a, rl.cz - (float)cur.box.lz);
+                    // byte address = base + 4*(iF + pS*iS + pZ*iZ); the magic-number bias of the three
+                    // float bit patterns is folded into the base
+                    const unsigned base = smem_u32(buf0 + stage * box_elems) - 4u * FT_MAGIC_BITS * (unsigned)(1 + pS + pZ);
+                    float part = 0.f, jf = 0.f;
+                    const int n = jb - ja + 1;
+#pragma unroll 2
+                    for (int j = 0; j < n; ++j, jf += 1.f) {
+                        const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
+                        const float qf = __fadd_rd(F, FT_MAGIC), qs = __fadd_rd(S, FT_MAGIC), qz = __fadd_rd(Z, FT_MAGIC);
+                        const float wf = F - (qf - FT_MAGIC), ws = S - (qs - FT_MAGIC), wz = Z - (qz - FT_MAGIC);
+                        const unsigned idx = __float_as_uint(qf) + (unsigned)pS * __float_as_uint(qs) +
+                                             (unsigned)pZ * __float_as_uint(qz);
+                        const unsigned a0 = base + 4u * idx, a1 = a0 + 4u * pS, a2 = a0 + 4u * pZ, a3 = a2 + 4u * pS;
+                        float v000, v100, v010, v110, v001, v101, v011, v111;
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
+                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v100) : "r"(a0));
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v010) : "r"(a1));
+                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v110) : "r"(a1));
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v001) : "r"(a2));
+                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v101) : "r"(a2));
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v011) : "r"(a3));
+                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v111) : "r"(a3));
+                        const float a00 = fmaf(wf, v100 - v000, v000), a10 = fmaf(wf, v110 - v010, v010);
+                        const float a01 = fmaf(wf, v101 - v001, v001), a11 = fmaf(wf, v111 - v011, v011);
+                        const float b0 = fmaf(ws, a10 - a00, a00), b1 = fmaf(ws, a11 - a01, a01);
+                        part += fmaf(wz, b1 - b0, b0);
+                    }
+                    total += part;
+                }
+            } else if (ja <= jb) {
+                // a chunk whose box does not fit even for one sample: read the volume directly
+                float part = 0.f;
+                for (int j = ja; j <= jb; ++j) {
+                    const float tau = fmaf((float)(j - k0), stepf, cur.tau_base);
+                    const float X = fmaf(r.bx, tau, r.cx), Y = fmaf(r.by, tau, r.cy), Z = fmaf(r.bz, tau, r.cz);
+                    const float fxf = floorf(X), fyf = floorf(Y), fzf = floorf(Z);
+                    const int ix = (int)fxf, iy = (int)fyf, iz = (int)fzf;
+                    const float wx = X - fxf, wy = Y - fyf, wz = Z - fzf;
+                    const float v000 = fetch0g(vol, g, ix, iy, iz), v100 = fetch0g(vol, g, ix + 1, iy, iz);
+                    const float v010 = fetch0g(vol, g, ix, iy + 1, iz), v110 = fetch0g(vol, g, ix + 1, iy + 1, iz);
+                    const float v001 = fetch0g(vol, g, ix, iy, iz + 1), v101 = fetch0g(vol, g, ix + 1, iy, iz + 1);
+                    const float v011 = fetch0g(vol, g, ix, iy + 1, iz + 1), v111 = fetch0g(vol, g, ix + 1, iy + 1, iz + 1);
+                    const float a00 = fmaf(wx, v100 - v000, v000), a10 = fmaf(wx, v110 - v010, v010);
+                    const float a01 = fmaf(wx, v101 - v001, v001), a11 = fmaf(wx, v111 - v011, v011);
+                    const float b0 = fmaf(wy, a10 - a00, a00), b1 = fmaf(wy, a11 - a01, a01);
+                    part += fmaf(wz, b1 - b0, b0);
+                }
+                total += part;
+            }
+            __syncthreads();                              // everyone is done with buffer `stage`
+            cur = nxt; k0 = kn; stage ^= 1;
+        }
+    }
+    if (valid) proj[((size_t)view * g.nv + iv) * g.nu + iu] = total * stepf;
+}
+
+// volT[z][x][y] = vol[z][y][x]
+__global__ void __launch_bounds__(256) transpose_vol_kernel(const float *__restrict__ v, float *__restrict__ vT, int nx, int ny) {
+    __shared__ float tile[32][33];
+    const size_t base = (size_t)blockIdx.z * nx * ny;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int x = x0 + threadIdx.x, y = y0 + j;
+        if (x < nx && y < ny) tile[j][threadIdx.x] = __ldg(v + base + (size_t)y * nx + x);
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int x = x0 + j, y = y0 + threadIdx.x;
+        if (x < nx && y < ny) vT[base + (size_t)x * ny + y] = tile[threadIdx.x][j];
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        else
+            (void)cudaGetLastError();
+    }
+    return fn;
+}
+
+// tensor map of a [n2][n1][n0] fp32 volume (n0 fastest) with a (b0, b1, b2) box, zero fill outside
+static bool make_map(CUtensorMap *m, const float *ptr, int n0, int n1, int n2, int b0, int b1, int b2) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)n0, (cuuint64_t)n1, (cuuint64_t)n2};
+    const cuuint64_t strides[2] = {(cuuint64_t)n0 * 4, (cuuint64_t)n0 * n1 * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(ptr), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// choose the box for this geometry (once, at create); fw_tma_ok = 0 when the TMA path cannot be used
+void plan_forward_tma(cbct_geometry *G) {
+    const cbct_geometry_desc &d = G->desc;
+    G->fw_tma_ok = 0;
+    if (d.nx % 4 || d.ny % 4) return;                            // TMA global strides must be multiples of 16 bytes
+    const double far = (d.sad + G->R) / d.sdd;
+    const double half_diag = 0.5 * std::sqrt((FT_TU * d.du) * (FT_TU * d.du) + (FT_TV * d.dv) * (FT_TV * d.dv));
+    const double psi = half_diag / d.sdd, vmin = std::fmin(d.dx, std::fmin(d.dy, d.dz));
+    const double margin = (d.sad + G->R) * 0.5 * psi * psi / vmin + 0.02;      // sphere-patch sagitta + rounding slack
+    if (margin > 2.0) return;
+    const double vxy = std::fmin(d.dx, d.dy);
+    const double wl = FT_TU * d.du * far / vxy, wv = FT_TV * d.dv * far;       // tile footprint: lateral (voxels), vertical (mm)
+    const double tilt = std::fmax(std::fabs(d.v0) + 0.5 * d.nv * d.dv, 1e-9) / d.sdd;   // |tan| of the steepest ray
+    const int kc_goal = 24;
+    const double travel = kc_goal * G->step / vxy;
+    const int bz = (int)std::ceil(wv / d.dz + kc_goal * G->step * tilt / d.dz + 2 * margin) + 3;
+    int bxy = (int)std::ceil(0.7072 * (wl + travel + wv * tilt / vxy) + 2 * margin) + 4 + 3;   // +3: 4-aligned box origin
+    bxy = std::max(16, (bxy + 3) & ~3);
+    if (bxy > 64 || bz > 32) return;
+    if ((size_t)2 * bxy * bxy * bz * 4 > 96 * 1024) return;
+    G->fw_b = bxy; G->fw_bz = bz; G->fw_margin = (float)margin;
+    if (cudaMalloc(&G->d_fw_volT, sizeof(float) * G->n_vox) != cudaSuccess) { (void)cudaGetLastError(); G->d_fw_volT = nullptr; return; }
+    G->workspace_bytes += sizeof(float) * G->n_vox;
+    static_assert(sizeof(CUtensorMap) <= sizeof(G->fw_map_y), "tensor map storage");
+    CUtensorMap m;
+    if (!make_map(&m, G->d_fw_volT, d.ny, d.nx, d.nz, bxy, bxy, bz)) return;
+    std::memcpy(G->fw_map_y, &m, sizeof(m));
+    if (cudaFuncSetAttribute(forward_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return;
+    }
+    G->fw_tma_ok = 1;
+}
+
+int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st) {
+    if (!G->fw_tma_ok || (reinterpret_cast<uintptr_t>(d_vol) & 15)) return CBCT_E_UNSUPPORTED;
+    const DevGeom &g = G->dg;
+    CUtensorMap mx, my;
+    if (!make_map(&mx, d_vol, g.nx, g.ny, g.nz, G->fw_b, G->fw_b, G->fw_bz)) return CBCT_E_UNSUPPORTED;
+    std::memcpy(&my, G->fw_map_y, sizeof(my));
+    {
+        dim3 block(32, 8), grid(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
+        transpose_vol_kernel<<<grid, block, 0, st>>>(d_vol, G->d_fw_volT, g.nx, g.ny);
+        CBCT_LAUNCH_CHECK();
+    }
+    const size_t smem = (size_t)2 * ((G->fw_b * G->fw_b * G->fw_bz + 31) & ~31) * 4;
+    dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), g.n_views);
+    forward_tma_kernel<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bz,
+                                                       getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+}  // namespace cbct

@@ -87,10 +87,14 @@ def test_forward_global_kernel_and_oversized_tiles(monkeypatch):
     shared-memory box (fine voxels under coarse pixels) go through the same parity bar."""
     f = syn.uniform_volume(ODD, 23)
     ref = op.forward(ODD, f.astype(np.float64))
-    monkeypatch.setenv("CBCT_FORWARD_IMPL", "global")
-    g, _ = gpu_forward(ODD, f)
+    for impl in ("global", "tiled"):
+        monkeypatch.setenv("CBCT_FORWARD_IMPL", impl)
+        g, _ = gpu_forward(ODD, f)
+        assert rel_l2_per_view(g, ref) <= TOL, impl
+        w1, _, f1, _ = syn.make_inputs(1, noisy=False)           # 4-divisible sizes: the same data the TMA path sees
+        g1, _ = gpu_forward(w1.geometry, f1)
+        assert rel_l2_per_view(g1, op.forward(w1.geometry, f1.astype(np.float64))) <= TOL, impl
     monkeypatch.delenv("CBCT_FORWARD_IMPL")
-    assert rel_l2_per_view(g, ref) <= TOL
     for vox, pix in ((0.25, 3.0), (0.6, 2.0), (1.0, 1.2)):
         G = syn.Geometry(96, 80, 24, vox, vox, 2 * vox, 40, 12, pix, pix, 1000.0, 1500.0, (0.1, 0.9, 2.4, 3.9),
                          step_mm=0.8 * vox)
