@@ -116,7 +116,7 @@ struct cbct_geometry {
     float *d_bp_projT;                  // P^T workspace: projections transposed to [view][iu][iv]
     cbct::BpTables bp;                  // P^T lookup tables (device pointers + constants)
     // forward TMA path (forward_tma.cu): box plan, y-fastest volume copy and its tensor map
-    int fw_tma_ok, fw_b, fw_bz;
+    int fw_tma_ok, fw_b, fw_bs, fw_bz;      // box: fw_b columns (= row pitch) x fw_bs rows x fw_bz planes
     float fw_margin;
     float *d_fw_volT;
     alignas(64) unsigned char fw_map_y[128];

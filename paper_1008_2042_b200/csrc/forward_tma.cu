@@ -59,7 +59,7 @@ struct Box3 { int lf, ls, lz; bool fits; };
 
 // origin of the box for samples tau_a..tau_b of the tile (AABB of the 4 corner rays at both ends grown by
 // `margin`), and whether its extents (+1 for the upper neighbour) fit the fixed box (bfs x bfs x bzz)
-__device__ __forceinline__ Box3 chunk_box(const RayL *corner, float tau_a, float tau_b, float margin, int bfs, int bzz) {
+__device__ __forceinline__ Box3 chunk_box(const RayL *corner, float tau_a, float tau_b, float margin, int bfs, int bss, int bzz) {
     float mnf = 1e30f, mns = 1e30f, mnz = 1e30f, mxf = -1e30f, mxs = -1e30f, mxz = -1e30f;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
@@ -77,20 +77,20 @@ __device__ __forceinline__ Box3 chunk_box(const RayL *corner, float tau_a, float
     // TMA: the innermost start coordinate must keep the global address 16-byte aligned -> multiple of 4
     b.lf = ((int)floorf(mnf - margin)) & ~3; b.ls = (int)floorf(mns - margin); b.lz = (int)floorf(mnz - margin);
     const int hf = (int)floorf(mxf + margin) + 1, hs = (int)floorf(mxs + margin) + 1, hz = (int)floorf(mxz + margin) + 1;
-    b.fits = (hf - b.lf + 1 <= bfs) && (hs - b.ls + 1 <= bfs) && (hz - b.lz + 1 <= bzz);
+    b.fits = (hf - b.lf + 1 <= bfs) && (hs - b.ls + 1 <= bss) && (hz - b.lz + 1 <= bzz);
     return b;
 }
 
 struct ChunkPlan { int kc; Box3 box; float tau_base; };
 
 __device__ __forceinline__ ChunkPlan plan_chunk(const DevGeom &g, const RayL *corner, int k0, int K1, float margin, int bfs,
-                                                int bzz) {
+                                                int bss, int bzz) {
     ChunkPlan p;
     p.tau_base = (float)(g.tau0 + (double)k0 * g.step);
     const float stepf = (float)g.step;
     int kc = min(FT_KCMAX, K1 - k0 + 1);
     for (;;) {
-        p.box = chunk_box(corner, p.tau_base, fmaf((float)(kc - 1), stepf, p.tau_base), margin, bfs, bzz);
+        p.box = chunk_box(corner, p.tau_base, fmaf((float)(kc - 1), stepf, p.tau_base), margin, bfs, bss, bzz);
         if (p.box.fits || kc == 1) break;
         kc = (kc > 8) ? (kc * 3) >> 2 : kc - 1;            // 64, 48, 36, 27, 20, 15, 11, 8, 7, ...
     }
@@ -106,17 +106,18 @@ __device__ __forceinline__ float fetch0g(const float *__restrict__ vol, const De
 __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
                                                                  const float *__restrict__ vol, float *__restrict__ proj,
-                                                                 float margin, int bfs, int bzz, int dbg) {
+                                                                 float margin, int bfs, int bss, int bzz, int dbg) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2];
     __shared__ RayL corner[4];
     __shared__ int s_klo, s_khi;
     float *buf0 = reinterpret_cast<float *>(smem_raw);
-    const int box_elems = (bfs * bfs * bzz + 31) & ~31;   // buffer stride: keeps the second buffer 128-byte aligned
-    const unsigned box_bytes = (unsigned)(bfs * bfs * bzz) * 4u;
+    const int box_elems = (bfs * bss * bzz + 31) & ~31;   // buffer stride: keeps the second buffer 128-byte aligned
+    const unsigned box_bytes = (unsigned)(bfs * bss * bzz) * 4u;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tu = lane & 15, tv = 2 * warp + (lane >> 4);
+    // a warp covers 8(u) x 4(v) pixels: <= 10 columns of the fast axis, <= 2 rows, <= 2 z-planes
+    const int tu = (warp & 1) * 8 + (lane & 7), tv = (warp >> 1) * 4 + (lane >> 3);
     const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = blockIdx.z;
     const bool valid = iu < g.nu && iv < g.nv;
 
@@ -165,11 +166,11 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
     const int K0 = s_klo, K1 = s_khi;
     const float stepf = (float)g.step;
     const float sF = rl.bf * stepf, sS = rl.bs * stepf, sZ = rl.bz * stepf;
-    const int pS = bfs, pZ = bfs * bfs;
+    const int pS = bfs, pZ = bfs * bss;
     float total = 0.f;
 
     if (K0 <= K1) {
-        ChunkPlan cur = plan_chunk(g, corner, K0, K1, margin, bfs, bzz);
+        ChunkPlan cur = plan_chunk(g, corner, K0, K1, margin, bfs, bss, bzz);
         if (tid == 0 && cur.box.fits && !(dbg & 1)) {
             mbar_expect_tx(smem_u32(&bars[0]), box_bytes);
             if (yfast) tma_load_3d(smem_u32(buf0), &map_y, cur.box.lf, cur.box.ls, cur.box.lz, smem_u32(&bars[0]));
@@ -181,7 +182,7 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
             const int kn = k0 + cur.kc;
             ChunkPlan nxt = cur;
             if (kn <= K1) {
-                nxt = plan_chunk(g, corner, kn, K1, margin, bfs, bzz);
+                nxt = plan_chunk(g, corner, kn, K1, margin, bfs, bss, bzz);
                 if (tid == 0 && nxt.box.fits && !(dbg & 1)) {          // the other buffer was released by the barrier below
                     const unsigned bar = smem_u32(&bars[stage ^ 1]);
                     mbar_expect_tx(bar, box_bytes);
@@ -320,17 +321,24 @@ void plan_forward_tma(cbct_geometry *G) {
     const double tilt = std::fmax(std::fabs(d.v0) + 0.5 * d.nv * d.dv, 1e-9) / d.sdd;   // |tan| of the steepest ray
     const int kc_goal = 24;
     const double travel = kc_goal * G->step / vxy;
-    const int bz = (int)std::ceil(wv / d.dz + kc_goal * G->step * tilt / d.dz + 2 * margin) + 3;
+    const int bz = (int)std::ceil(wv / d.dz + kc_goal * G->step * tilt / d.dz + 2 * margin) + 2;
     int bxy = (int)std::ceil(0.7072 * (wl + travel + wv * tilt / vxy) + 2 * margin) + 4 + 3;   // +3: 4-aligned box origin
-    bxy = std::max(16, (bxy + 3) & ~3);
-    if (bxy > 64 || bz > 32) return;
-    if ((size_t)2 * bxy * bxy * bz * 4 > 96 * 1024) return;
-    G->fw_b = bxy; G->fw_bz = bz; G->fw_margin = (float)margin;
+    // Bank = (F + pitch*S + pitch*rows*Z) mod 32.  A warp's 8x4 pixels span <= 10 columns F, <= 2 rows S and
+    // <= 2 planes Z, so a pitch of +-8 (mod 32) and a plane pitch of 16 (mod 32) keep its 32 lanes in distinct
+    // banks (or on the same word) for every view direction: pitch in {24, 40, 56}, rows = 2 (mod 4).
+    const int need_f = bxy, need_s = bxy - 3;
+    int bf = 0;
+    for (int cand : {24, 40, 56})
+        if (cand >= need_f) { bf = cand; break; }
+    if (!bf || bz > 32) return;
+    const int bs = ((std::max(need_s, 14) - 2 + 3) / 4) * 4 + 2;
+    if ((size_t)2 * bf * bs * bz * 4 > 96 * 1024) return;
+    G->fw_b = bf; G->fw_bs = bs; G->fw_bz = bz; G->fw_margin = (float)margin;
     if (cudaMalloc(&G->d_fw_volT, sizeof(float) * G->n_vox) != cudaSuccess) { (void)cudaGetLastError(); G->d_fw_volT = nullptr; return; }
     G->workspace_bytes += sizeof(float) * G->n_vox;
     static_assert(sizeof(CUtensorMap) <= sizeof(G->fw_map_y), "tensor map storage");
     CUtensorMap m;
-    if (!make_map(&m, G->d_fw_volT, d.ny, d.nx, d.nz, bxy, bxy, bz)) return;
+    if (!make_map(&m, G->d_fw_volT, d.ny, d.nx, d.nz, bf, bs, bz)) return;
     std::memcpy(G->fw_map_y, &m, sizeof(m));
     if (cudaFuncSetAttribute(forward_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
         (void)cudaGetLastError();
@@ -343,16 +351,16 @@ int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj
     if (!G->fw_tma_ok || (reinterpret_cast<uintptr_t>(d_vol) & 15)) return CBCT_E_UNSUPPORTED;
     const DevGeom &g = G->dg;
     CUtensorMap mx, my;
-    if (!make_map(&mx, d_vol, g.nx, g.ny, g.nz, G->fw_b, G->fw_b, G->fw_bz)) return CBCT_E_UNSUPPORTED;
+    if (!make_map(&mx, d_vol, g.nx, g.ny, g.nz, G->fw_b, G->fw_bs, G->fw_bz)) return CBCT_E_UNSUPPORTED;
     std::memcpy(&my, G->fw_map_y, sizeof(my));
     {
         dim3 block(32, 8), grid(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
         transpose_vol_kernel<<<grid, block, 0, st>>>(d_vol, G->d_fw_volT, g.nx, g.ny);
         CBCT_LAUNCH_CHECK();
     }
-    const size_t smem = (size_t)2 * ((G->fw_b * G->fw_b * G->fw_bz + 31) & ~31) * 4;
+    const size_t smem = (size_t)2 * ((G->fw_b * G->fw_bs * G->fw_bz + 31) & ~31) * 4;
     dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), g.n_views);
-    forward_tma_kernel<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bz,
+    forward_tma_kernel<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz,
                                                        getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
