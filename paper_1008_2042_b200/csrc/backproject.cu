@@ -203,26 +203,50 @@ __global__ void __launch_bounds__(MAXT, MINB) backproject_cell_kernel(BpTables P
 }
 
 // voxel (x,y,z) = step * sum over the 8 cells (x-dx, y-dy, z-dz) of their corner (dx,dy,dz) accumulator.
-// One thread per (x,y) column walking z: lanes are neighbours in x (coalesced float stores), and the
-// z-fastest partials are re-used from L1 along the walk.
-__global__ void __launch_bounds__(128) backproject_combine_kernel(const float *__restrict__ partial, float *__restrict__ vol,
+// The partials are z-fastest, the volume x-fastest: a CTA takes 32 x-neighbouring columns of one y, its
+// warps read whole z-runs (coalesced), sum the 8 contributions in a fixed order in registers, and the
+// tile is transposed through shared memory so that the volume is written with coalesced rows.
+__global__ void __launch_bounds__(256) backproject_combine_kernel(const float *__restrict__ partial, float *__restrict__ vol,
                                                                   int nx, int ny, int nz, float stepf) {
+    extern __shared__ float tile[];                     // [32][pitch], pitch odd
+    const int pitch = nz | 1;
+    const int x0 = blockIdx.x * 32, y = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nzc = nz + 1;
+    const size_t ncell = (size_t)(nx + 1) * (ny + 1) * nzc;
+    for (int j = warp; j < 32; j += 8) {
+        const int x = x0 + j;
+        if (x >= nx) break;
+        for (int z = lane; z < nz; z += 32) {
+            float acc = 0.f;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const int dx = c & 1, dy = (c >> 1) & 1, dz = c >> 2;
+                acc += __ldg(partial + (size_t)c * ncell + ((size_t)(y - dy + 1) * (nx + 1) + (x - dx + 1)) * nzc + (z - dz + 1));
+            }
+            tile[j * pitch + z] = acc * stepf;
+        }
+    }
+    __syncthreads();
+    const int x = x0 + lane;
+    if (x < nx)
+        for (int z = warp; z < nz; z += 8) vol[((size_t)z * ny + y) * nx + x] = tile[lane * pitch + z];
+}
+
+// fall-back for volumes too tall for the shared-memory tile: one thread per (x,y) column walking z
+__global__ void __launch_bounds__(128) backproject_combine_simple_kernel(const float *__restrict__ partial,
+                                                                         float *__restrict__ vol, int nx, int ny, int nz,
+                                                                         float stepf) {
     const int x = blockIdx.x * 32 + threadIdx.x, y = blockIdx.y * 4 + threadIdx.y;
     if (x >= nx || y >= ny) return;
     const int nzc = nz + 1;
     const size_t ncell = (size_t)(nx + 1) * (ny + 1) * nzc;
-    const float *col[4];
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        const int dx = c & 1, dy = c >> 1;
-        col[c] = partial + ((size_t)(y - dy + 1) * (nx + 1) + (x - dx + 1)) * nzc + (size_t)c * ncell;
-    }
     for (int z = 0; z < nz; ++z) {
         float acc = 0.f;
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
-            const int dz = c >> 2;
-            acc += __ldg(col[c & 3] + (size_t)dz * 4 * ncell + (z - dz + 1));
+            const int dx = c & 1, dy = (c >> 1) & 1, dz = c >> 2;
+            acc += __ldg(partial + (size_t)c * ncell + ((size_t)(y - dy + 1) * (nx + 1) + (x - dx + 1)) * nzc + (z - dz + 1));
         }
         vol[((size_t)z * ny + y) * nx + x] = acc * stepf;
     }
@@ -350,8 +374,14 @@ int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol
         CBCT_LAUNCH_CHECK();
     }
     {
-        dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4));
-        backproject_combine_kernel<<<grid, block, 0, st>>>(G->d_bp_partial, d_vol, g.nx, g.ny, g.nz, (float)G->step);
+        const size_t smem = sizeof(float) * 32 * (size_t)(g.nz | 1);
+        if (smem <= 48 * 1024) {
+            dim3 grid(cdiv(g.nx, 32), g.ny);
+            backproject_combine_kernel<<<grid, 256, smem, st>>>(G->d_bp_partial, d_vol, g.nx, g.ny, g.nz, (float)G->step);
+        } else {
+            dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4));
+            backproject_combine_simple_kernel<<<grid, block, 0, st>>>(G->d_bp_partial, d_vol, g.nx, g.ny, g.nz, (float)G->step);
+        }
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;

@@ -103,6 +103,8 @@ __device__ __forceinline__ float fetch0g(const float *__restrict__ vol, const De
     return __ldg(vol + ((size_t)iz * g.ny + iy) * g.nx + ix);
 }
 
+// BF, BS > 0: box pitches known at compile time (neighbour loads use immediate offsets); 0: run-time pitches
+template <int BF, int BS>
 __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
                                                                  const float *__restrict__ vol, float *__restrict__ proj,
@@ -110,6 +112,7 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2];
     __shared__ RayL corner[4];
+    __shared__ ChunkPlan plans[2];
     __shared__ int s_klo, s_khi;
     float *buf0 = reinterpret_cast<float *>(smem_raw);
     const int box_elems = (bfs * bss * bzz + 31) & ~31;   // buffer stride: keeps the second buffer 128-byte aligned
@@ -166,29 +169,35 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
     const int K0 = s_klo, K1 = s_khi;
     const float stepf = (float)g.step;
     const float sF = rl.bf * stepf, sS = rl.bs * stepf, sZ = rl.bz * stepf;
-    const int pS = bfs, pZ = bfs * bss;
+    const int pS = BF > 0 ? BF : bfs, pZ = BF > 0 ? BF * BS : bfs * bss;
     float total = 0.f;
 
     if (K0 <= K1) {
-        ChunkPlan cur = plan_chunk(g, corner, K0, K1, margin, bfs, bss, bzz);
-        if (tid == 0 && cur.box.fits && !(dbg & 1)) {
-            mbar_expect_tx(smem_u32(&bars[0]), box_bytes);
-            if (yfast) tma_load_3d(smem_u32(buf0), &map_y, cur.box.lf, cur.box.ls, cur.box.lz, smem_u32(&bars[0]));
-            else tma_load_3d(smem_u32(buf0), &map_x, cur.box.lf, cur.box.ls, cur.box.lz, smem_u32(&bars[0]));
+        // thread 0 plans every chunk (box origin, length), issues its TMA copy and publishes the plan
+        if (tid == 0) {
+            const ChunkPlan p0 = plan_chunk(g, corner, K0, K1, margin, bfs, bss, bzz);
+            plans[0] = p0;
+            if (p0.box.fits && !(dbg & 1)) {
+                mbar_expect_tx(smem_u32(&bars[0]), box_bytes);
+                if (yfast) tma_load_3d(smem_u32(buf0), &map_y, p0.box.lf, p0.box.ls, p0.box.lz, smem_u32(&bars[0]));
+                else tma_load_3d(smem_u32(buf0), &map_x, p0.box.lf, p0.box.ls, p0.box.lz, smem_u32(&bars[0]));
+            }
         }
+        __syncthreads();
         unsigned phase0 = 0, phase1 = 0;
         int k0 = K0, stage = 0;
         while (k0 <= K1) {
+            const ChunkPlan cur = plans[stage];
             const int kn = k0 + cur.kc;
-            ChunkPlan nxt = cur;
-            if (kn <= K1) {
-                nxt = plan_chunk(g, corner, kn, K1, margin, bfs, bss, bzz);
-                if (tid == 0 && nxt.box.fits && !(dbg & 1)) {          // the other buffer was released by the barrier below
+            if (tid == 0 && kn <= K1) {                  // the other buffer and plan slot were released by the barrier below
+                const ChunkPlan nx_ = plan_chunk(g, corner, kn, K1, margin, bfs, bss, bzz);
+                plans[stage ^ 1] = nx_;
+                if (nx_.box.fits && !(dbg & 1)) {
                     const unsigned bar = smem_u32(&bars[stage ^ 1]);
                     mbar_expect_tx(bar, box_bytes);
                     const unsigned dst = smem_u32(buf0 + (stage ^ 1) * box_elems);
-                    if (yfast) tma_load_3d(dst, &map_y, nxt.box.lf, nxt.box.ls, nxt.box.lz, bar);
-                    else tma_load_3d(dst, &map_x, nxt.box.lf, nxt.box.ls, nxt.box.lz, bar);
+                    if (yfast) tma_load_3d(dst, &map_y, nx_.box.lf, nx_.box.ls, nx_.box.lz, bar);
+                    else tma_load_3d(dst, &map_x, nx_.box.lf, nx_.box.ls, nx_.box.lz, bar);
                 }
             }
             const int ja = max(k0, klo), jb = min(kn - 1, khi);
@@ -213,16 +222,28 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                         const float wf = F - (qf - FT_MAGIC), ws = S - (qs - FT_MAGIC), wz = Z - (qz - FT_MAGIC);
                         const unsigned idx = __float_as_uint(qf) + (unsigned)pS * __float_as_uint(qs) +
                                              (unsigned)pZ * __float_as_uint(qz);
-                        const unsigned a0 = base + 4u * idx, a1 = a0 + 4u * pS, a2 = a0 + 4u * pZ, a3 = a2 + 4u * pS;
+                        const unsigned a0 = base + 4u * idx;
                         float v000, v100, v010, v110, v001, v101, v011, v111;
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
-                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v100) : "r"(a0));
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v010) : "r"(a1));
-                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v110) : "r"(a1));
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v001) : "r"(a2));
-                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v101) : "r"(a2));
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v011) : "r"(a3));
-                        asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v111) : "r"(a3));
+                        if constexpr (BF > 0) {
+                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
+                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v100) : "r"(a0));
+                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v010) : "r"(a0), "n"(4 * BF));
+                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v110) : "r"(a0), "n"(4 * BF + 4));
+                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v001) : "r"(a0), "n"(4 * BF * BS));
+                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v101) : "r"(a0), "n"(4 * BF * BS + 4));
+                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v011) : "r"(a0), "n"(4 * BF * BS + 4 * BF));
+                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v111) : "r"(a0), "n"(4 * BF * BS + 4 * BF + 4));
+                        } else {
+                            const unsigned a1 = a0 + 4u * pS, a2 = a0 + 4u * pZ, a3 = a2 + 4u * pS;
+                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
+                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v100) : "r"(a0));
+                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v010) : "r"(a1));
+                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v110) : "r"(a1));
+                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v001) : "r"(a2));
+                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v101) : "r"(a2));
+                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v011) : "r"(a3));
+                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v111) : "r"(a3));
+                        }
                         const float a00 = fmaf(wf, v100 - v000, v000), a10 = fmaf(wf, v110 - v010, v010);
                         const float a01 = fmaf(wf, v101 - v001, v001), a11 = fmaf(wf, v111 - v011, v011);
                         const float b0 = fmaf(ws, a10 - a00, a00), b1 = fmaf(ws, a11 - a01, a01);
@@ -250,8 +271,8 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                 }
                 total += part;
             }
-            __syncthreads();                              // everyone is done with buffer `stage`
-            cur = nxt; k0 = kn; stage ^= 1;
+            __syncthreads();                              // everyone is done with buffer `stage`; next plan is visible
+            k0 = kn; stage ^= 1;
         }
     }
     if (valid) proj[((size_t)view * g.nv + iv) * g.nu + iu] = total * stepf;
@@ -306,6 +327,17 @@ static bool make_map(CUtensorMap *m, const float *ptr, int n0, int n1, int n2, i
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+typedef void (*TmaKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, float *, float, int, int, int, int);
+static TmaKernel tma_kernel_ptr(int bf, int bs) {
+    if (bf == 24 && bs == 22) return forward_tma_kernel<24, 22>;
+    if (bf == 40 && bs == 30) return forward_tma_kernel<40, 30>;
+    if (bf == 40 && bs == 38) return forward_tma_kernel<40, 38>;
+    if (bf == 56 && bs == 46) return forward_tma_kernel<56, 46>;
+    if (bf == 56 && bs == 54) return forward_tma_kernel<56, 54>;
+    return nullptr;
+}
+static const void *tma_kernel_for(int bf, int bs) { return reinterpret_cast<const void *>(tma_kernel_ptr(bf, bs)); }
+
 // choose the box for this geometry (once, at create); fw_tma_ok = 0 when the TMA path cannot be used
 void plan_forward_tma(cbct_geometry *G) {
     const cbct_geometry_desc &d = G->desc;
@@ -327,11 +359,11 @@ void plan_forward_tma(cbct_geometry *G) {
     // <= 2 planes Z, so a pitch of +-8 (mod 32) and a plane pitch of 16 (mod 32) keep its 32 lanes in distinct
     // banks (or on the same word) for every view direction: pitch in {24, 40, 56}, rows = 2 (mod 4).
     const int need_f = bxy, need_s = bxy - 3;
-    int bf = 0;
-    for (int cand : {24, 40, 56})
-        if (cand >= need_f) { bf = cand; break; }
+    int bf = 0, bs = 0;
+    const int menu[][2] = {{24, 22}, {40, 30}, {40, 38}, {56, 46}, {56, 54}};   // compiled instantiations
+    for (auto &m : menu)
+        if (m[0] >= need_f && m[1] >= need_s) { bf = m[0]; bs = m[1]; break; }
     if (!bf || bz > 32) return;
-    const int bs = ((std::max(need_s, 14) - 2 + 3) / 4) * 4 + 2;
     if ((size_t)2 * bf * bs * bz * 4 > 96 * 1024) return;
     G->fw_b = bf; G->fw_bs = bs; G->fw_bz = bz; G->fw_margin = (float)margin;
     if (cudaMalloc(&G->d_fw_volT, sizeof(float) * G->n_vox) != cudaSuccess) { (void)cudaGetLastError(); G->d_fw_volT = nullptr; return; }
@@ -340,7 +372,8 @@ void plan_forward_tma(cbct_geometry *G) {
     CUtensorMap m;
     if (!make_map(&m, G->d_fw_volT, d.ny, d.nx, d.nz, bf, bs, bz)) return;
     std::memcpy(G->fw_map_y, &m, sizeof(m));
-    if (cudaFuncSetAttribute(forward_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
+    const void *kern = tma_kernel_for(bf, bs);
+    if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
         (void)cudaGetLastError();
         return;
     }
@@ -360,7 +393,9 @@ int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj
     }
     const size_t smem = (size_t)2 * ((G->fw_b * G->fw_bs * G->fw_bz + 31) & ~31) * 4;
     dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), g.n_views);
-    forward_tma_kernel<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz,
+    TmaKernel kern = tma_kernel_ptr(G->fw_b, G->fw_bs);
+    if (!kern) return CBCT_E_UNSUPPORTED;
+    kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz,
                                                        getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
