@@ -210,19 +210,20 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                     const float F0 = fmaf(rl.bf, tau_a, rl.cf - (float)cur.box.lf);
                     const float S0 = fmaf(rl.bs, tau_a, rl.cs - (float)cur.box.ls);
                     const float Z0 = fmaf(rl.bz, tau_a, rl.cz - (float)cur.box.lz);
-                    // byte address = base + 4*(iF + pS*iS + pZ*iZ); the magic-number bias of the three
-                    // float bit patterns is folded into the base
-                    const unsigned base = smem_u32(buf0 + stage * box_elems) - 4u * FT_MAGIC_BITS * (unsigned)(1 + pS + pZ);
+                    // byte address = base + 4*(iF + pS*iS + pZ*iZ); the element index is formed exactly in fp32
+                    // (< 2^24) from the floors that the fractions need anyway, then converted once
+                    const unsigned base_r = smem_u32(buf0 + stage * box_elems);
+                    const float pSf = (float)pS, pZf = (float)pZ;
                     float part = 0.f, jf = 0.f;
                     const int n = jb - ja + 1;
 #pragma unroll 2
                     for (int j = 0; j < n; ++j, jf += 1.f) {
                         const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
                         const float qf = __fadd_rd(F, FT_MAGIC), qs = __fadd_rd(S, FT_MAGIC), qz = __fadd_rd(Z, FT_MAGIC);
-                        const float wf = F - (qf - FT_MAGIC), ws = S - (qs - FT_MAGIC), wz = Z - (qz - FT_MAGIC);
-                        const unsigned idx = __float_as_uint(qf) + (unsigned)pS * __float_as_uint(qs) +
-                                             (unsigned)pZ * __float_as_uint(qz);
-                        const unsigned a0 = base + 4u * idx;
+                        const float rf = qf - FT_MAGIC, rs = qs - FT_MAGIC, rz = qz - FT_MAGIC;      // floors, exact
+                        const float wf = F - rf, ws = S - rs, wz = Z - rz;
+                        const unsigned idx = (unsigned)__float2int_rn(fmaf(rz, pZf, fmaf(rs, pSf, rf)));
+                        const unsigned a0 = base_r + 4u * idx;
                         float v000, v100, v010, v110, v001, v101, v011, v111;
                         if constexpr (BF > 0) {
                             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
