@@ -152,29 +152,23 @@ def main():
     ap.add_argument("--kernels-only", action="store_true", help="run P, P^T, fused TF 3x and exit (for ncu)")
     args = ap.parse_args()
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1008_2042_b200 import replicas
+    rank, world, local_rank = replicas.world()
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
 
     import torch
-    import torch.distributed as dist
     from paper_1008_2042_b200 import binding as cb
     from paper_1008_2042_b200 import synthetic as syn
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    replicas.init("nccl", torch.device("cuda", local_rank))
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier("cuda")
 
     w = syn.workload(args.workload)
     G = w.geometry
@@ -263,11 +257,7 @@ def main():
     prof = cb.profile_end()
     launches = cb.launch_count() - launches0
     clocks = sampler.stop() if sampler else None
-    step_ms = float(np.sum(ms))
-    if world > 1:
-        t = torch.tensor([step_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        step_ms = float(t.item())
+    step_ms = replicas.max_over_ranks(float(np.sum(ms)), "cuda")
     value = world * samples_per_step * args.steps / (step_ms * 1e-3) / 1e9
 
     # ---- end-to-end arm (host buffers through the C ABI) -----------------------------------------
@@ -276,11 +266,7 @@ def main():
     barrier()
     ms_e2e = timed(step_host, args.steps)
     barrier()
-    e2e_ms = float(np.sum(ms_e2e))
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = replicas.max_over_ranks(float(np.sum(ms_e2e)), "cuda")
     e2e_value = world * samples_per_step * args.steps / (e2e_ms * 1e-3) / 1e9
 
     # ---- standalone kernels (context numbers) -----------------------------------------------------
@@ -293,8 +279,7 @@ def main():
     ms_tf = float(np.median(timed(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True), 5)))
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        replicas.shutdown()
         return
 
     peaks = load_peaks()
@@ -345,8 +330,7 @@ def main():
                    wall_s_timed_region=t_wall,
                    paper_context="paper: ~2.7-3.5 s per P+P^T pair, ~5 min full recon on Tesla C1060 (PAPER.md:23, :402)"))
     print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.shutdown()
 
 
 if __name__ == "__main__":
