@@ -150,6 +150,7 @@ def main():
     ap.add_argument("--workload", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernels-only", action="store_true", help="run P, P^T, fused TF 3x and exit (for ncu)")
+    ap.add_argument("--no-full-recon", action="store_true", help="skip the one-off 3-level 5/10/15 reconstruction timing")
     args = ap.parse_args()
 
     from paper_1008_2042_b200 import replicas
@@ -278,6 +279,22 @@ def main():
     ms_pt = float(np.median(timed(lambda: geom.backproject(d_g, d_tmp), 5)))
     ms_tf = float(np.median(timed(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True), 5)))
 
+    # ---- the paper's full reconstruction, end to end (context number; 3 levels, 5/10/15) ----
+    full_recon_s = None
+    if rank == 0 and not args.no_full_recon:
+        del d_alpha                                            # 2 GB of three-call coefficients no longer needed
+        rec3 = cb.Recon(G, 3)
+        rec3.run(d_g, d_f, [1, 1, 1], N_CGLS, MU, True)       # warm-up
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        rec3.run(d_g, d_f, [5, 10, 15], N_CGLS, MU, True)
+        b.record()
+        torch.cuda.synchronize()
+        full_recon_s = a.elapsed_time(b) * 1e-3
+        rrms = float(torch.linalg.vector_norm(d_f - d_vol) / torch.linalg.vector_norm(d_vol))
+        rec3.close()
+
     if rank != 0:
         replicas.shutdown()
         return
@@ -326,6 +343,10 @@ def main():
                    p_gsamples_s=geom.n_samples / ms_p / 1e6, pt_gsamples_s=geom.n_samples / ms_pt / 1e6,
                    s_per_cgls_iter=(ms_p + ms_pt) * 1e-3 + 0.0,
                    s_per_cgls_iter_in_step=(ms_f / max(n_f, 1) + ms_b / max(n_b, 1)) * 1e-3,
+                   full_recon_s=full_recon_s,
+                   full_recon="3-level multigrid, 5/10/15 A2 outer iterations, n_cgls=3, mu=5e-4, device-resident "
+                              "(PAPER.md:288 recipe; paper: ~5 min on Tesla C1060)",
+                   full_recon_rrms_vs_phantom=(rrms if full_recon_s is not None else None),
                    tf_fused_gbs=2 * geom.n_vox * 4 / ms_tf / 1e6, hbm_peak_gbs=peaks["hbm_gbs"],
                    wall_s_timed_region=t_wall,
                    paper_context="paper: ~2.7-3.5 s per P+P^T pair, ~5 min full recon on Tesla C1060 (PAPER.md:23, :402)"))

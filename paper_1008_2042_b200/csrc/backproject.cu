@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(256) transpose_proj_kernel(const float *__rest
     }
 }
 
-template <int MAXT, int MINB>
+template <int MAXT, int MINB, bool ZCLIP>
 __global__ void __launch_bounds__(MAXT, MINB) backproject_cell_kernel(BpTables P, int nx, int ny, int nz, int nu, int nv,
                                                                int n_views, int K, int xb, const float *__restrict__ projT,
                                                                float *__restrict__ partial) {
@@ -160,12 +160,24 @@ __global__ void __launch_bounds__(MAXT, MINB) backproject_cell_kernel(BpTables P
             const float4 *pp = P.pixT + (iu * nv + iv0);
             const float *gp = pv + (iu * nv + iv0);
             const float2 *rp = P.rows + iv0;
-            for (int iv = iv0; iv <= iv1; ++iv, ++pp, ++gp, ++rp) {
-                const float2 rw = __ldg(rp);                                           // vz, 1/vz
-                const float4 t = __ldg(pp);                                            // 1/L, q, L
-                const float gval = __ldg(gp);                                          // all three loads in flight together
-                const float rz0 = az * rw.y, rz1 = bz * rw.y;
-                const float rlo = fmaxf(rin, fminf(rz0, rz1)), rhi = fminf(rout, fmaxf(rz0, rz1));
+            if (iv0 > iv1) continue;
+            // software pipeline: the three loads of row iv+1 are issued before row iv is processed
+            float2 rw_n = __ldg(rp);
+            float4 t_n = __ldg(pp);
+            float g_n = __ldg(gp);
+            for (int iv = iv0; iv <= iv1; ++iv) {
+                const float2 rw = rw_n;                                                // vz, 1/vz
+                const float4 t = t_n;                                                  // 1/L, q, L
+                const float gval = g_n;
+                const int adv = iv < iv1 ? 1 : 0;                                      // stay in range on the last row
+                pp += adv; gp += adv; rp += adv;
+                rw_n = __ldg(rp); t_n = __ldg(pp); g_n = __ldg(gp);
+                // z clip of the k-range: only worth its instructions when rays are steep against flat cells
+                float rlo = rin, rhi = rout;
+                if constexpr (ZCLIP) {
+                    const float rz0 = az * rw.y, rz1 = bz * rw.y;
+                    rlo = fmaxf(rin, fminf(rz0, rz1)); rhi = fminf(rout, fmaxf(rz0, rz1));
+                }
                 const float sl = t.z * inv_step;
                 const int ka = max(0, (int)ceilf(fmaf(rlo, sl, k_lo_off)));
                 const int kb = min(K - 1, (int)floorf(fmaf(rhi, sl, k_hi_off)));
@@ -364,13 +376,16 @@ int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol
         if (nzc > 512) return CBCT_E_UNSUPPORTED;   // taller volumes: use CBCT_BACKPROJECT_IMPL=gather
         const int threads = ((xb * nzc + 31) / 32) * 32;
         dim3 grid(cdiv(g.nx + 1, xb), g.ny + 1);
-        const char *var = getenv("CBCT_BP_VARIANT");                  // "4": 48-register build, 4 CTAs/SM (experiments)
-        if (threads <= 320 && var && var[0] == '4')
-            backproject_cell_kernel<320, 4><<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K,
-                                                                       xb, G->d_bp_projT, G->d_bp_partial);
-        else
-            backproject_cell_kernel<512, 2><<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, g.K,
-                                                                       xb, G->d_bp_projT, G->d_bp_partial);
+        // z travel of the steepest ray across one cell's x,y chord, in cells: small -> skip the z clip
+        const cbct_geometry_desc &d = G->desc;
+        const double tan_max = (std::fabs(d.v0) + 0.5 * d.nv * d.dv) / d.sdd;
+        const bool zclip = tan_max * 1.4143 * std::fmax(d.dx, d.dy) / d.dz > 0.25;
+#define CBCT_BP_LAUNCH(MAXT, MINB, ZC)                                                                              \
+    backproject_cell_kernel<MAXT, MINB, ZC><<<grid, threads, 0, st>>>(G->bp, g.nx, g.ny, g.nz, g.nu, g.nv, g.n_views, \
+                                                                      g.K, xb, G->d_bp_projT, G->d_bp_partial)
+        if (threads <= 320) { if (zclip) CBCT_BP_LAUNCH(320, 3, true); else CBCT_BP_LAUNCH(320, 3, false); }
+        else { if (zclip) CBCT_BP_LAUNCH(512, 2, true); else CBCT_BP_LAUNCH(512, 2, false); }
+#undef CBCT_BP_LAUNCH
         CBCT_LAUNCH_CHECK();
     }
     {

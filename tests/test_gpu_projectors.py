@@ -208,6 +208,19 @@ def test_backproject_gather_kernel_cross_check(monkeypatch):
     assert rel_l2(f_cell, f_gather.astype(np.float64)) <= TOL
 
 
+def test_flat_cells_steep_rays():
+    """Flat voxels under a tall detector (steep rays): exercises the z-clipped variant of the
+    cell-driven backprojector and tall shared-memory boxes in the forward projector."""
+    G = syn.Geometry(24, 20, 40, 4.0, 4.0, 0.5, 28, 64, 5.0, 8.0, 1000.0, 1500.0, (0.2, 1.3, 2.9, 4.1, 5.6),
+                     oz=3.0, step_mm=0.4)
+    y = syn.uniform_projections(G, 28) - 0.2
+    f, _ = gpu_back(G, y)
+    assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL
+    x = syn.uniform_volume(G, 29)
+    g, _ = gpu_forward(G, x)
+    assert rel_l2_per_view(g, op.forward(G, x.astype(np.float64))) <= TOL
+
+
 def test_backproject_axis_parallel_rays_and_fine_steps():
     """Rays exactly parallel to a grid axis (central pixel at 0 and 90 degrees, odd detector) and a
     sampling step much finer / coarser than the voxel."""
