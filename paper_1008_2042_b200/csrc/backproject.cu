@@ -350,7 +350,11 @@ int build_bp_tables(cbct_geometry *G) {
 int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
     const DevGeom &g = G->dg;
     ProfScope prof(PROF_BACK, st);
-    const char *impl = getenv("CBCT_BACKPROJECT_IMPL");              // "gather" forces the per-voxel kernel (tests)
+    // CBCT_BACKPROJECT_IMPL = "gather" | "cell" | "scatter" forces one implementation (tests); default: scatter
+    // (backproject_tma.cu) when the geometry supports it, else the cell-driven kernel below
+    const char *impl = getenv("CBCT_BACKPROJECT_IMPL");
+    if (impl && impl[0] == 's') return launch_backproject_tma(G, d_proj, d_vol, st);
+    if (!impl && G->bt_ok) return launch_backproject_tma(G, d_proj, d_vol, st);
     if (impl && impl[0] == 'g') {
         dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4), g.nz);
         backproject_gather_kernel<<<grid, block, 0, st>>>(g, d_proj, d_vol);

@@ -1,0 +1,375 @@
+// backproject_tma.cu -- f = P^T g, the sm_100a fast path of cbct_backproject (include/cbct.h).
+// The exact transpose of forward_tma.cu, organised as its mirror image (PAPER.md:211 names the obstacle --
+// write conflicts of a ray-driven scatter -- which is removed here by hardware, not by changing the operator):
+//   * a CTA owns the same 16(u) x 16(v) pixel tile of one view and marches the same chunks of the global
+//     t-grid, with the same fp32 sample positions and trilinear weights as the forward kernel;
+//   * instead of reading 8 voxels per sample from a TMA-loaded box it ADDS g * weight to the 8 voxels of an
+//     accumulator box in shared memory.  The accumulators are 32-bit FIXED POINT: shared-memory integer
+//     atomics (ATOMS.ADD) run at the rate of plain shared stores on sm_100a, whereas a float atomicAdd on shared
+//     memory compiles to a compare-and-swap loop (3x slower, measured).  Integer addition is associative, so
+//     the result does not depend on the order of the atomics: P^T is deterministic;
+//   * a finished box is added to a global int32 accumulator volume by ONE TMA tensor reduction
+//     (cp.reduce.async.bulk.tensor.3d ... .add, element type s32); elements outside the volume are skipped
+//     by the TMA unit, which is the transpose of the forward kernel's zero fill.  Two boxes alternate, so the
+//     reduction of one chunk overlaps the scattering of the next;
+//   * a last pass converts the accumulators to fp32 (x step / scale) with coalesced float4 stores.
+// Fixed point: every ray value is scaled by S = 2^qb / max|g| (max|g| reduced on the device per call), each
+// contribution S g w is rounded to the nearest integer by one FFMA onto 1.5 * 2^23, and qb is chosen at
+// geometry-create so that the largest possible voxel sum of a view group stays below 2^31.  The rounding
+// error per contribution is uniform in +-max|g| / 2^(qb+1) (qb = 21 at the paper-size config): relative to the
+// result that is ~1e-6 * max|g| / rms(g) -- an order of magnitude below the fp32 rounding of the weights
+// themselves for any input whose peak is within ~30 rms (projections, CGLS residuals).
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+#include "tma_common.cuh"
+
+namespace cbct {
+
+constexpr float BT_ROUND = 12582912.0f;          // 1.5 * 2^23: x + BT_ROUND holds round(x) in its low mantissa bits, |x| < 2^22
+constexpr int BT_ROUND_BITS = 0x4B400000;
+
+__device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap *map, int c0, int c1, int c2, unsigned src) {
+    asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
+                 "r"(src), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// integer nearest to c = a*b (|c| < 2^22), in one FFMA + one IADD
+__device__ __forceinline__ int round_mul(float a, float b) { return __float_as_int(fmaf(a, b, BT_ROUND)) - BT_ROUND_BITS; }
+__device__ __forceinline__ void red_s32(unsigned addr, int v) { asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
+template <int OFF>
+__device__ __forceinline__ void red_s32_off(unsigned addr, int v) {
+    asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(v) : "memory");
+}
+
+// max |g| as the bit pattern of a non-negative float (orders like an unsigned integer); *out zeroed before
+__global__ void __launch_bounds__(256) absmax_kernel(const float *__restrict__ g, long long n, unsigned *out) {
+    float m = 0.f;
+    const long long n4 = n >> 2;
+    const float4 *g4 = reinterpret_cast<const float4 *>(g);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) {
+        const float4 v = __ldg(g4 + i);
+        m = fmaxf(m, fmaxf(fmaxf(fabsf(v.x), fabsf(v.y)), fmaxf(fabsf(v.z), fabsf(v.w))));
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (n & 3)) m = fmaxf(m, fabsf(__ldg(g + (n4 << 2) + threadIdx.x)));
+    unsigned b = __float_as_uint(m);
+    b = __reduce_max_sync(0xffffffffu, b);
+    if ((threadIdx.x & 31) == 0 && b) atomicMax(out, b);
+}
+
+// Bank conflicts decide the speed of this kernel (it is bound by shared-memory wavefronts: two lanes of one
+// ATOMS that fall on the same bank -- same word or not -- cost one extra wavefront each).  Lane layouts and
+// box pitches were searched with a CPU model of the cfg-4 geometry that reproduces the ncu wavefront counts:
+//   LM 0: a warp = 8(u) x 4(v) pixels, the lane group of row r works 2r samples ahead of row 0 (its samples are
+//         one voxel further along the ray = one box row = +8 banks), box pitch = 8 (mod 32), plane pitch = 0
+//         (mod 32): 2.2 wavefronts per ATOMS;
+//   LM 1: a warp = 16(u) x 2(v), rows 8 apart (their samples lie in different z-planes), no skew, the forward
+//         kernel's box (pitch 8, plane pitch 16 mod 32): 2.9 wavefronts per ATOMS (model) / 2.96 (ncu).
+// LM 1 is the default until LM 0 (CBCT_BT_LANES=0 at geometry-create) has been timed on the device.
+// The order in which a thread visits the samples of a chunk is free: integer sums do not depend on it.
+template <int BF, int BS, int LM>
+__global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
+                                                                         const __grid_constant__ CUtensorMap map_y,
+                                                                         const float *__restrict__ proj, int *__restrict__ acc_x,
+                                                                         const unsigned *__restrict__ absmax_bits, float two_qb,
+                                                                         int view0, float margin, int bzz, int dbg) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ RayL corner[4];
+    __shared__ ChunkPlan plans[2];
+    __shared__ int s_klo, s_khi;
+    constexpr int bfs = BF, bss = BS;
+    int *buf0 = reinterpret_cast<int *>(smem_raw);
+    const int box_words = bfs * bss * bzz;
+    const int box_elems = (box_words + 31) & ~31;          // buffer stride: keeps the second buffer 128-byte aligned
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int tu, tv;
+    if constexpr (LM == 0) { tu = (warp & 1) * 8 + (lane & 7); tv = (warp >> 1) * 4 + (lane >> 3); }
+    else { tu = lane & 15; tv = warp + 8 * (lane >> 4); }
+    const int skew = LM == 0 ? 2 * (lane >> 3) : 0;
+    const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = view0 + blockIdx.z;
+    const bool valid = iu < g.nu && iv < g.nv;
+
+    const double2 cs = g.view_cs[view];
+    const bool yfast = fabs(cs.x) > fabs(cs.y);             // same orientation rule as forward_tma_kernel
+
+    RayF r;
+    double b[3], c[3];
+    ray_setup(g, view, iv, iu, r, b[0], b[1], b[2], c[0], c[1], c[2]);
+    int klo = 0x7fffffff, khi = -1;
+    if (valid) {
+        const double hi[3] = {(double)g.nx, (double)g.ny, (double)g.nz};
+        double tin = -1e300, tout = 1e300;
+        bool miss = false;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (b[a] == 0.0) { miss |= (c[a] <= -1.0 || c[a] >= hi[a]); continue; }
+            const double inv = 1.0 / b[a];
+            double t1 = (-1.0 - c[a]) * inv, t2 = (hi[a] - c[a]) * inv;
+            if (t1 > t2) { const double t = t1; t1 = t2; t2 = t; }
+            tin = fmax(tin, t1); tout = fmin(tout, t2);
+        }
+        if (!miss && tout > tin) {
+            const long long a = (long long)ceil((tin - g.tau0) / g.step), e = (long long)floor((tout - g.tau0) / g.step);
+            klo = (int)max(a, 0LL); khi = (int)min(e, (long long)g.K - 1);
+            if (khi < klo) { klo = 0x7fffffff; khi = -1; }
+        }
+    }
+    RayL rl;
+    rl.cf = yfast ? r.cy : r.cx; rl.cs = yfast ? r.cx : r.cy; rl.cz = r.cz;
+    rl.bf = yfast ? r.by : r.bx; rl.bs = yfast ? r.bx : r.by; rl.bz = r.bz;
+
+    // ray value in fixed-point units: |gs| <= 2^qb
+    const float amax = __uint_as_float(__ldg(absmax_bits));
+    const float scale = amax > 0.f ? two_qb / amax : 0.f;
+    const float gs = valid ? __ldg(proj + ((size_t)view * g.nv + iv) * g.nu + iu) * scale : 0.f;
+
+    if (tid == 0) { s_klo = 0x7fffffff; s_khi = -1; }
+    if ((tu == 0 || tu == FT_TU - 1) && (tv == 0 || tv == FT_TV - 1)) corner[(tv ? 2 : 0) + (tu ? 1 : 0)] = rl;
+    {   // both accumulator boxes start at zero
+        int4 *z = reinterpret_cast<int4 *>(buf0);
+        for (int i = tid; i < (2 * box_elems) >> 2; i += FT_THREADS) z[i] = make_int4(0, 0, 0, 0);
+    }
+    __syncthreads();
+    {
+        const int wlo = __reduce_min_sync(0xffffffffu, klo), whi = __reduce_max_sync(0xffffffffu, khi);
+        if (lane == 0) { atomicMin(&s_klo, wlo); atomicMax(&s_khi, whi); }
+    }
+    __syncthreads();
+    const int K0 = s_klo, K1 = s_khi;
+    if (K0 > K1) return;
+    const float stepf = (float)g.step;
+    const float sF = rl.bf * stepf, sS = rl.bs * stepf, sZ = rl.bz * stepf;
+    constexpr int pS = BF, pZ = BF * BS;
+
+    if (tid == 0) plans[0] = plan_chunk(g, corner, K0, K1, margin, bfs, bss, bzz);
+    __syncthreads();
+    int k0 = K0, stage = 0;
+    bool first = true;
+    while (k0 <= K1) {
+        const ChunkPlan cur = plans[stage];
+        const int kn = k0 + cur.kc;
+        if (tid == 0 && kn <= K1) plans[stage ^ 1] = plan_chunk(g, corner, kn, K1, margin, bfs, bss, bzz);
+        const int ja = max(k0, klo), jb = min(kn - 1, khi);
+        if (cur.box.fits) {
+            if (ja <= jb && !(dbg & 2)) {
+                const float tau_a = fmaf((float)(ja - k0), stepf, cur.tau_base);
+                const float F0 = fmaf(rl.bf, tau_a, rl.cf - (float)cur.box.lf);
+                const float S0 = fmaf(rl.bs, tau_a, rl.cs - (float)cur.box.ls);
+                const float Z0 = fmaf(rl.bz, tau_a, rl.cz - (float)cur.box.lz);
+                const unsigned base_r = smem_u32(buf0 + stage * box_elems);
+                const float pSf = (float)pS, pZf = (float)pZ;
+                const int n = jb - ja + 1;
+                const float nf = (float)n;
+                float jf = (float)(skew < n ? skew : skew % n);        // start `skew` samples ahead, wrap around at n
+#pragma unroll 2
+                for (int j = 0; j < n; ++j) {
+                    // identical position / floor / fraction arithmetic to forward_tma_kernel
+                    const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
+                    const float qf = __fadd_rd(F, FT_MAGIC), qs = __fadd_rd(S, FT_MAGIC), qz = __fadd_rd(Z, FT_MAGIC);
+                    const float rf = qf - FT_MAGIC, rs = qs - FT_MAGIC, rz = qz - FT_MAGIC;
+                    const float wf = F - rf, ws = S - rs, wz = Z - rz;
+                    const unsigned idx = (unsigned)__float2int_rn(fmaf(rz, pZf, fmaf(rs, pSf, rf)));
+                    const unsigned a0 = base_r + 4u * idx;
+                    // transposed lerp tree: split gs along z, then the slow axis, then the fast axis
+                    const float g1 = gs * wz, g0 = gs - g1;
+                    const float g01 = g0 * ws, g00 = g0 - g01, g11 = g1 * ws, g10 = g1 - g11;
+                    const float of = 1.f - wf;
+                    red_s32_off<0>(a0, round_mul(g00, of));
+                    red_s32_off<4>(a0, round_mul(g00, wf));
+                    red_s32_off<4 * BF>(a0, round_mul(g01, of));
+                    red_s32_off<4 * BF + 4>(a0, round_mul(g01, wf));
+                    red_s32_off<4 * BF * BS>(a0, round_mul(g10, of));
+                    red_s32_off<4 * BF * BS + 4>(a0, round_mul(g10, wf));
+                    red_s32_off<4 * BF * BS + 4 * BF>(a0, round_mul(g11, of));
+                    red_s32_off<4 * BF * BS + 4 * BF + 4>(a0, round_mul(g11, wf));
+                    jf += 1.f;
+                    if (jf >= nf) jf -= nf;
+                }
+            }
+            fence_async_smem();                           // my shared-memory writes -> visible to the TMA unit
+        } else if (ja <= jb) {
+            // a chunk whose box does not fit even for one sample: integer atomics straight on the x-fastest volume
+            for (int j = ja; j <= jb; ++j) {
+                const float tau = fmaf((float)(j - k0), stepf, cur.tau_base);
+                const float X = fmaf(r.bx, tau, r.cx), Y = fmaf(r.by, tau, r.cy), Z = fmaf(r.bz, tau, r.cz);
+                const float fxf = floorf(X), fyf = floorf(Y), fzf = floorf(Z);
+                const int ix = (int)fxf, iy = (int)fyf, iz = (int)fzf;
+                const float wx = X - fxf, wy = Y - fyf, wz = Z - fzf;
+#pragma unroll
+                for (int cc = 0; cc < 8; ++cc) {
+                    const int x = ix + (cc & 1), y = iy + ((cc >> 1) & 1), z = iz + (cc >> 2);
+                    if ((unsigned)x >= (unsigned)g.nx || (unsigned)y >= (unsigned)g.ny || (unsigned)z >= (unsigned)g.nz) continue;
+                    const float w = ((cc & 1) ? wx : 1.f - wx) * ((cc & 2) ? wy : 1.f - wy) * ((cc & 4) ? wz : 1.f - wz);
+                    atomicAdd(acc_x + ((size_t)(z + bzz) * (g.ny + bss) + (y + bss)) * (g.nx + bfs) + (x + bfs), round_mul(gs, w));
+                }
+            }
+        }
+        if (tid == 0) bulk_wait_read0();                  // the other box's reduction (issued one chunk ago) has read it
+        __syncthreads();                                  // A: everyone finished scattering into box `stage`
+        if (tid == 0 && cur.box.fits && !(dbg & 1)) {
+            // The accumulator volumes carry a low-side margin of one box (a tensor reduction may not start at a
+            // negative coordinate; elements beyond the high side are skipped by the TMA unit).  A box that starts
+            // below the margin, or beyond the high side, lies entirely outside the volume: nothing to add.
+            const unsigned src = smem_u32(buf0 + stage * box_elems);
+            const int oF = cur.box.lf + bfs, oS = cur.box.ls + bss, oZ = cur.box.lz + bzz;
+            const int nF = (yfast ? g.ny : g.nx) + bfs, nS = (yfast ? g.nx : g.ny) + bss, nZ = g.nz + bzz;
+            if (oF >= 0 && oS >= 0 && oZ >= 0 && oF < nF && oS < nS && oZ < nZ) {
+                if (yfast) tma_reduce_add_3d(&map_y, oF, oS, oZ, src);
+                else tma_reduce_add_3d(&map_x, oF, oS, oZ, src);
+                bulk_commit();
+            }
+        }
+        if (!first && kn <= K1) {                         // clear the other box for the next chunk
+            int4 *z = reinterpret_cast<int4 *>(buf0 + (stage ^ 1) * box_elems);
+            for (int i = tid; i < box_elems >> 2; i += FT_THREADS) z[i] = make_int4(0, 0, 0, 0);
+        }
+        first = false;
+        __syncthreads();                                  // B: the cleared box and the next plan are visible
+        k0 = kn; stage ^= 1;
+    }
+    if (tid == 0) bulk_wait0();                           // shared memory must outlive the last reduction
+}
+
+// vol[z][y][x] (+)= (acc_x[z][y][x] + acc_y[z][x][y]) * step * max|g| / 2^qb; 32x32 tiles, the y-fastest accumulator is
+// transposed through shared memory so that every global access is a coalesced row
+// (both accumulators carry a low-side margin of one box: pf x ps x pz elements, fast axis first)
+__global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y,
+                                                                   float *__restrict__ vol, int nx, int ny, int pf, int ps, int pz,
+                                                                   const unsigned *__restrict__ absmax_bits, float step_over_two_qb,
+                                                                   int accumulate) {
+    __shared__ int tile[32][33];
+    const size_t base = (size_t)blockIdx.z * nx * ny;
+    const size_t base_x = ((size_t)(blockIdx.z + pz) * (ny + ps) + ps) * (nx + pf) + pf;     // acc_x[z+pz][ps][pf]
+    const size_t base_y = ((size_t)(blockIdx.z + pz) * (nx + ps) + ps) * (ny + pf) + pf;     // acc_y[z+pz][ps][pf]
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    const float k = __uint_as_float(__ldg(absmax_bits)) * step_over_two_qb;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int y = y0 + threadIdx.x, x = x0 + j;
+        if (x < nx && y < ny) tile[j][threadIdx.x] = __ldg(acc_y + base_y + (size_t)x * (ny + pf) + y);
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int x = x0 + threadIdx.x, y = y0 + j;
+        if (x < nx && y < ny) {
+            const size_t o = base + (size_t)y * nx + x;
+            const float v = (float)(__ldg(acc_x + base_x + (size_t)y * (nx + pf) + x) + tile[threadIdx.x][j]) * k;
+            vol[o] = accumulate ? vol[o] + v : v;
+        }
+    }
+}
+
+typedef void (*ScatterKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, int *, const unsigned *, float, int,
+                              float, int, int);
+static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm) {
+#define CBCT_SK(F, S, L) if (bf == F && bs == S && lm == L) return backproject_scatter_kernel<F, S, L>;
+    CBCT_SK(24, 24, 0) CBCT_SK(40, 32, 0) CBCT_SK(40, 40, 0) CBCT_SK(56, 48, 0) CBCT_SK(56, 56, 0)      // plane pitch = 0 (mod 32)
+    CBCT_SK(24, 22, 1) CBCT_SK(40, 30, 1) CBCT_SK(40, 38, 1) CBCT_SK(56, 46, 1) CBCT_SK(56, 54, 1)      // the forward kernel's boxes
+#undef CBCT_SK
+    return nullptr;
+}
+
+void free_backproject_tma(cbct_geometry *G) {
+    cudaFree(G->d_bt_acc);
+    cudaFree(G->d_bt_absmax);
+    G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr; G->bt_ok = 0;
+}
+
+// decide whether the scatter path runs for this geometry; needs the forward TMA box plan (same boxes)
+void plan_backproject_tma(cbct_geometry *G) {
+    const cbct_geometry_desc &d = G->desc;
+    G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
+    if (!G->fw_tma_ok) return;
+    // lane layout (see the kernel): CBCT_BT_LANES=0 selects the skewed 8x4 layout, whose box is the forward kernel's
+    // with the row count rounded up to a multiple of 4 (plane pitch = 0 mod 32); default 1 = 16x2, forward's box
+    const char *lm_env = getenv("CBCT_BT_LANES");
+    G->bt_lm = (lm_env && atoi(lm_env) == 0) ? 0 : 1;
+    G->bt_b = G->fw_b; G->bt_bz = G->fw_bz; G->bt_bs = G->bt_lm == 0 ? (G->fw_bs + 3) & ~3 : G->fw_bs;
+    if ((size_t)2 * G->bt_b * G->bt_bs * G->bt_bz * 4 > 100 * 1024) return;
+    // Largest possible sum of trilinear weights landing on one voxel from ONE view: the continuum density of
+    // samples (rays per area at the nearest depth / step) times the voxel volume, times the worst-case
+    // excess of a sum of hat samples over its mean when the sampling pitch exceeds the voxel pitch, x 1.5.
+    const double near = d.sdd / G->t_min, far = (d.sad + G->R) / d.sdd;
+    const double mean_w = d.dx * d.dy * d.dz * near * near / (d.du * d.dv * G->step);
+    const double su = std::fmax(1.0, d.du * far / std::fmin(d.dx, d.dy)), sv = std::fmax(1.0, d.dv * far / d.dz);
+    const double st = std::fmax(1.0, G->step / std::fmin(d.dx, std::fmin(d.dy, d.dz)));
+    const double w_view = 1.5 * mean_w * su * sv * st;
+    // views per group and fixed-point bits: group * w_view * 2^qb < 2^31, qb <= 22 (the rounding trick's range)
+    int qb = 21, group = d.n_views;
+    const auto cap = [&](int bits) { return std::ldexp(1.0, 31 - bits) / w_view; };
+    if (cap(22) >= d.n_views) qb = 22;
+    else if (cap(21) >= d.n_views) qb = 21;
+    else {
+        qb = 21;
+        while (qb > 12 && cap(qb) < 1.0) --qb;
+        if (cap(qb) < 1.0) return;
+        group = (int)std::fmin((double)d.n_views, std::floor(cap(qb)));
+    }
+    G->bt_qb = qb; G->bt_group = group;
+    const size_t n_acc = (size_t)(d.nx + G->bt_b) * (d.ny + G->bt_bs) * (d.nz + G->bt_bz);      // x-fastest, with margins
+    const size_t n_acc_y = (size_t)(d.ny + G->bt_b) * (d.nx + G->bt_bs) * (d.nz + G->bt_bz);    // y-fastest
+    G->bt_acc_y_off = (n_acc + 31) & ~(size_t)31;
+    G->bt_acc_elems = G->bt_acc_y_off + n_acc_y;
+    if (cudaMalloc(&G->d_bt_acc, sizeof(int) * G->bt_acc_elems) != cudaSuccess ||
+        cudaMalloc(&G->d_bt_absmax, sizeof(unsigned)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        free_backproject_tma(G);
+        return;
+    }
+    G->workspace_bytes += sizeof(int) * G->bt_acc_elems + sizeof(unsigned);
+    CUtensorMap mx, my;
+    if (!make_map(&mx, G->d_bt_acc, d.nx + G->bt_b, d.ny + G->bt_bs, d.nz + G->bt_bz, G->bt_b, G->bt_bs, G->bt_bz,
+                  CU_TENSOR_MAP_DATA_TYPE_INT32) ||
+        !make_map(&my, G->d_bt_acc + G->bt_acc_y_off, d.ny + G->bt_b, d.nx + G->bt_bs, d.nz + G->bt_bz, G->bt_b, G->bt_bs, G->bt_bz,
+                  CU_TENSOR_MAP_DATA_TYPE_INT32)) {
+        free_backproject_tma(G);
+        return;
+    }
+    std::memcpy(G->bt_map_x, &mx, sizeof(mx));
+    std::memcpy(G->bt_map_y, &my, sizeof(my));
+    ScatterKernel k = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm);
+    if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) !=
+                  cudaSuccess) {
+        (void)cudaGetLastError();
+        free_backproject_tma(G);
+        return;
+    }
+    G->bt_ok = 1;
+}
+
+int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
+    if (!G->bt_ok) return CBCT_E_UNSUPPORTED;
+    const DevGeom &g = G->dg;
+    CUtensorMap mx, my;
+    std::memcpy(&mx, G->bt_map_x, sizeof(mx));
+    std::memcpy(&my, G->bt_map_y, sizeof(my));
+    ScatterKernel kern = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm);
+    if (!kern) return CBCT_E_UNSUPPORTED;
+    CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_absmax, 0, sizeof(unsigned), st));
+    absmax_kernel<<<592, 256, 0, st>>>(d_proj, (long long)G->n_rays, G->d_bt_absmax);
+    CBCT_LAUNCH_CHECK();
+    const size_t smem = (size_t)2 * ((G->bt_b * G->bt_bs * G->bt_bz + 31) & ~31) * 4;
+    const float two_qb = (float)std::ldexp(1.0, G->bt_qb);
+    const int dbg = getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0;
+    for (int v0 = 0; v0 < g.n_views; v0 += G->bt_group) {
+        const int nv_ = std::min(G->bt_group, g.n_views - v0);
+        CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_acc, 0, sizeof(int) * G->bt_acc_elems, st));
+        dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), nv_);
+        kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_proj, G->d_bt_acc, G->d_bt_absmax, two_qb, v0, G->fw_margin, G->bt_bz, dbg);
+        CBCT_LAUNCH_CHECK();
+        dim3 fb(32, 8), fg(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
+        backproject_finalize_kernel<<<fg, fb, 0, st>>>(G->d_bt_acc, G->d_bt_acc + G->bt_acc_y_off, d_vol, g.nx, g.ny, G->bt_b, G->bt_bs,
+                                                       G->bt_bz, G->d_bt_absmax,
+                                                       (float)(G->step / std::ldexp(1.0, G->bt_qb)), v0 > 0 ? 1 : 0);
+        CBCT_LAUNCH_CHECK();
+    }
+    return CBCT_OK;
+}
+
+}  // namespace cbct

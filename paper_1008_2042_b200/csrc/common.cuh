@@ -120,6 +120,15 @@ struct cbct_geometry {
     float fw_margin;
     float *d_fw_volT;
     alignas(64) unsigned char fw_map_y[128];
+    // P^T scatter path (backproject_tma.cu): int32 accumulator volumes (x-fastest, then y-fastest), max|g|, fixed-point plan
+    int bt_b, bt_bs, bt_bz;                 // accumulator box (row pitch bt_b, bt_bs rows, bt_bz planes)
+    int bt_lm;                              // lane layout of the scatter kernel (template parameter LM)
+    int bt_ok, bt_qb, bt_group;             // 2^bt_qb = fixed-point unit per max|g|; views per accumulation group
+    int *d_bt_acc;
+    size_t bt_acc_y_off, bt_acc_elems;      // element offset of the y-fastest accumulator, total elements
+    unsigned *d_bt_absmax;
+    alignas(64) unsigned char bt_map_x[128];
+    alignas(64) unsigned char bt_map_y[128];
     size_t workspace_bytes;
 };
 
@@ -138,6 +147,9 @@ int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cu
 int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
 void plan_forward_tma(cbct_geometry *g);     // decides whether/how the TMA forward kernel runs for this geometry
 int launch_forward_tma(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
+void plan_backproject_tma(cbct_geometry *g); // after plan_forward_tma: same boxes, int32 accumulators
+void free_backproject_tma(cbct_geometry *g);
+int launch_backproject_tma(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
 int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
 void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,

@@ -165,6 +165,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
     G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr; G->d_fw_volT = nullptr; G->fw_tma_ok = 0;
+    G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
     G->bp = BpTables{};
     G->workspace_bytes = 0;
 
@@ -192,6 +193,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     g.view_cs = G->d_view_cs;
 
     plan_forward_tma(G);
+    plan_backproject_tma(G);
     {
         const int st_bp = build_bp_tables(G);
         if (st_bp != CBCT_OK) { cbct_geometry_destroy(G); return st_bp; }
@@ -220,6 +222,7 @@ extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     cudaFree(G->d_ws_vol);
     cudaFree(G->d_ws_proj);
     free_bp_tables(G);
+    free_backproject_tma(G);
     cudaFree(G->d_fw_volT);
     (void)cudaGetLastError();
     delete G;
