@@ -102,6 +102,12 @@ __global__ void __launch_bounds__(128) backproject_gather_kernel(DevGeom g, cons
 // v-fastest (transposed) copies so that those lanes touch neighbouring addresses.
 // ------------------------------------------------------------------------------------------------
 constexpr float BP_EPS = 0.02f;
+// The clipping arithmetic (r-slabs from the fp32 tables) and the membership test (fp32 sample positions) round
+// differently; for a ray that grazes a cell face or corner a position error of 1e-5 voxel moves the crossing by
+// many samples.  Clipping therefore uses the cell grown by BP_GROW voxels on every side and accepts an (almost)
+// empty in-plane chord; membership is still decided by the positions alone.  (Found with the scatter kernel:
+// without this, 1e-8 of the samples at cfg 4 were skipped.)
+constexpr float BP_GROW = 1e-3f, BP_R_EPS = 1e-5f;
 
 // gT[view][iu][iv] = g[view][iv][iu]
 __global__ void __launch_bounds__(256) transpose_proj_kernel(const float *__restrict__ g, float *__restrict__ gT, int nu,
@@ -129,7 +135,7 @@ __global__ void __launch_bounds__(MAXT, MINB) backproject_cell_kernel(BpTables P
     const int ix = blockIdx.x * xb + xr - 1, iy = (int)blockIdx.y - 1, iz = zc - 1;
     if (xr >= xb || ix > nx - 1) return;
     const float fix = (float)ix, fiy = (float)iy, fiz = (float)iz;
-    const float az = fiz - P.Kz, bz = az + 1.f;
+    const float az = fiz - P.Kz - BP_GROW, bz = az + (1.f + 2.f * BP_GROW);
     float a000 = 0.f, a100 = 0.f, a010 = 0.f, a110 = 0.f, a001 = 0.f, a101 = 0.f, a011 = 0.f, a111 = 0.f;
     const float inv_step = P.inv_step, stepf = P.stepf, tau0f = P.tau0f;
     const float k_lo_off = -(P.t0 * P.inv_step) - P.k_eps, k_hi_off = -(P.t0 * P.inv_step) + P.k_eps;
@@ -147,10 +153,10 @@ __global__ void __launch_bounds__(MAXT, MINB) backproject_cell_kernel(BpTables P
         const float *pv = projT + (size_t)view * nv * nu;
         for (int iu = iu0; iu <= iu1; ++iu) {
             const float4 w0 = __ldg(reinterpret_cast<const float4 *>(vu + iu));        // Ax Ay Wx Wy
-            const float rx0 = (fix - V.Kx) * w0.z, rx1 = rx0 + w0.z;
-            const float ry0 = (fiy - V.Ky) * w0.w, ry1 = ry0 + w0.w;
+            const float rx0 = (fix - V.Kx - BP_GROW) * w0.z, rx1 = fmaf(1.f + 2.f * BP_GROW, w0.z, rx0);
+            const float ry0 = (fiy - V.Ky - BP_GROW) * w0.w, ry1 = fmaf(1.f + 2.f * BP_GROW, w0.w, ry0);
             const float rin = fmaxf(fminf(rx0, rx1), fminf(ry0, ry1)), rout = fminf(fmaxf(rx0, rx1), fmaxf(ry0, ry1));
-            if (!(rin < rout) || !(rin > 0.f)) continue;
+            if (!(rin < rout + BP_R_EPS) || !(rin > 0.f)) continue;
             const float2 w1 = __ldg(reinterpret_cast<const float2 *>(vu + iu) + 2);    // Gx Gy
             const float i_in = __frcp_rn(rin), i_out = __frcp_rn(rout);
             const float vzmin = fminf(az * i_in, az * i_out), vzmax = fmaxf(bz * i_in, bz * i_out);
