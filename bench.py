@@ -307,8 +307,13 @@ def main():
     f_clk = peaks["sm_max_mhz"] * 1e6
     peak_tinstr = N_SM * LANES_PER_CLK_PER_SM * f_clk / 1e12
     achieved_tinstr = geom.n_samples * INSTR_PER_SAMPLE / (dom_ms * 1e-3) / 1e12
+    # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` captures (profiles/README.md),
+    # cfg 4 only: P = forward_tma_kernel (r1_kernels_full.csv), P^T = scatter kernel, both view groups (r1_scatter_full.csv)
+    ncu_traffic = {("forward", 4): 1.851507e9 + 35.917e6, ("backproject", 4): (439.53e6 + 84.42e6) + (2.635912e9 + 0.169432e9)}
     roofline = dict(bound="alu", kernel=f"cbct_{dom}", achieved=achieved_tinstr, peak=peak_tinstr, unit="Tinstr/s",
-                    frac=achieved_tinstr / peak_tinstr, traffic=None,
+                    frac=achieved_tinstr / peak_tinstr, traffic=ncu_traffic.get((dom, args.workload)),
+                    traffic_unit="DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum); algorithmic HBM bytes "
+                                 "are 105e6 per launch, the kernel is not HBM bound",
                     algorithmic=f"{geom.n_samples} samples x {INSTR_PER_SAMPLE:.0f} thread-instr/sample per launch",
                     launch_ms=dom_ms, gsamples_s=geom.n_samples / (dom_ms * 1e-3) / 1e9,
                     peak_source=f"148 SM x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)",
