@@ -94,8 +94,20 @@ int cbct_geometry_info(const cbct_geometry *geom, int64_t *n_vox, int64_t *n_ray
 int cbct_forward(const cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
 
 /* f = P^T g, the exact matrix transpose of cbct_forward ("f = P^T g"; north_star),
- * voxel-driven and deterministic (no atomics).  d_proj: n_views*nv*nu, d_vol: nx*ny*nz. */
+ * deterministic (bit-identical from call to call).  d_proj: n_views*nv*nu, d_vol: nx*ny*nz, finite values.
+ * Where nx and ny are multiples of 4 and the sampling box fits shared memory the transpose is evaluated
+ * ray-driven with fixed-point shared-memory accumulators (error per contribution <= max|g| / 2^(qb+1), see
+ * cbct_backproject_fixed_point_plan); otherwise voxel-driven in fp32 without atomics. */
 int cbct_backproject(const cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
+
+/* Host arithmetic only (no device needed): the fixed-point plan cbct_backproject uses for this geometry.
+ *   max_weight_sum_per_view: upper bound on the sum of trilinear weights one voxel receives from one view;
+ *   qb: contributions are rounded to multiples of max|g| / 2^qb;
+ *   views_per_group: views accumulated in int32 before conversion to fp32
+ *                    (views_per_group * max_weight_sum_per_view * 2^qb < 2^31, so the sums cannot wrap).
+ * Any out pointer may be NULL.  CBCT_E_INVALID as cbct_geometry_create; CBCT_E_UNSUPPORTED if no plan exists. */
+int cbct_backproject_fixed_point_plan(const cbct_geometry_desc *desc, int32_t *qb, int32_t *views_per_group,
+                                      double *max_weight_sum_per_view);
 
 /* Host-buffer variants (used for end-to-end timing): copy h_in -> device workspace, run, copy the
  * result to h_out, all on `stream`; the caller synchronises the stream.  Pinned host memory makes

@@ -23,6 +23,7 @@ EXPORTS = [
     "cbct_profile_begin", "cbct_profile_end",
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
+    "cbct_backproject_fixed_point_plan",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
@@ -77,6 +78,8 @@ def lib():
                                      C.POINTER(C.c_size_t)]
     for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host"):
         getattr(L, name).argtypes = [vp, fp, fp, vp]
+    L.cbct_backproject_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                                    C.POINTER(C.c_double)]
     L.cbct_cgls_create.argtypes = [vp, C.POINTER(vp)]
     L.cbct_cgls_destroy.argtypes = [vp]
     L.cbct_cgls_init.argtypes = [vp, fp, fp, fp, fp, vp]
@@ -164,6 +167,15 @@ def make_desc(geom):
                      geom.nu, geom.nv, geom.du, geom.dv, geom.u0, geom.v0, geom.sad, geom.sdd,
                      len(ang), ang.ctypes.data_as(C.POINTER(C.c_double)), float(getattr(geom, "step_mm", 0.0)))
     return d, ang
+
+
+def backproject_fixed_point_plan(geom):
+    """(qb, views_per_group, max_weight_sum_per_view) of cbct_backproject for this geometry; host only."""
+    d, keep = make_desc(geom)
+    qb, grp, w = C.c_int32(), C.c_int32(), C.c_double()
+    _check(lib().cbct_backproject_fixed_point_plan(C.byref(d), C.byref(qb), C.byref(grp), C.byref(w)),
+           "cbct_backproject_fixed_point_plan")
+    return qb.value, grp.value, w.value
 
 
 class Geometry:

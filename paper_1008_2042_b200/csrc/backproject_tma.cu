@@ -275,6 +275,32 @@ static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm) {
     return nullptr;
 }
 
+// Fixed-point plan of the scatter kernel (host arithmetic only; exported as cbct_backproject_fixed_point_plan).
+// w_view bounds the sum of trilinear weights one voxel can receive from ONE view: the continuum density of
+// samples (rays per area at the nearest depth, / step) times the voxel volume, times the worst-case excess of a
+// sum of hat samples over its mean when a sampling pitch exceeds the voxel pitch, times 1.5.  Then
+// views_per_group * w_view * 2^qb < 2^31 with qb <= 22 (the range of the rounding trick).
+bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int *qb_out, int *group_out, double *w_view_out) {
+    const double t_min = d.sad - R;
+    const double near = d.sdd / t_min, far = (d.sad + R) / d.sdd;
+    const double mean_w = d.dx * d.dy * d.dz * near * near / (d.du * d.dv * step);
+    const double su = std::fmax(1.0, d.du * far / std::fmin(d.dx, d.dy)), sv = std::fmax(1.0, d.dv * far / d.dz);
+    const double st = std::fmax(1.0, step / std::fmin(d.dx, std::fmin(d.dy, d.dz)));
+    const double w_view = 1.5 * mean_w * su * sv * st;
+    int qb = 21, group = d.n_views;
+    const auto cap = [&](int bits) { return std::ldexp(1.0, 31 - bits) / w_view; };
+    if (cap(22) >= d.n_views) qb = 22;
+    else if (cap(21) >= d.n_views) qb = 21;
+    else {
+        qb = 21;
+        while (qb > 12 && cap(qb) < 1.0) --qb;
+        if (cap(qb) < 1.0) return false;
+        group = (int)std::fmin((double)d.n_views, std::floor(cap(qb)));
+    }
+    *qb_out = qb; *group_out = group; *w_view_out = w_view;
+    return true;
+}
+
 void free_backproject_tma(cbct_geometry *G) {
     cudaFree(G->d_bt_acc);
     cudaFree(G->d_bt_absmax);
@@ -292,25 +318,9 @@ void plan_backproject_tma(cbct_geometry *G) {
     G->bt_lm = (lm_env && atoi(lm_env) == 0) ? 0 : 1;
     G->bt_b = G->fw_b; G->bt_bz = G->fw_bz; G->bt_bs = G->bt_lm == 0 ? (G->fw_bs + 3) & ~3 : G->fw_bs;
     if ((size_t)2 * G->bt_b * G->bt_bs * G->bt_bz * 4 > 100 * 1024) return;
-    // Largest possible sum of trilinear weights landing on one voxel from ONE view: the continuum density of
-    // samples (rays per area at the nearest depth / step) times the voxel volume, times the worst-case
-    // excess of a sum of hat samples over its mean when the sampling pitch exceeds the voxel pitch, x 1.5.
-    const double near = d.sdd / G->t_min, far = (d.sad + G->R) / d.sdd;
-    const double mean_w = d.dx * d.dy * d.dz * near * near / (d.du * d.dv * G->step);
-    const double su = std::fmax(1.0, d.du * far / std::fmin(d.dx, d.dy)), sv = std::fmax(1.0, d.dv * far / d.dz);
-    const double st = std::fmax(1.0, G->step / std::fmin(d.dx, std::fmin(d.dy, d.dz)));
-    const double w_view = 1.5 * mean_w * su * sv * st;
-    // views per group and fixed-point bits: group * w_view * 2^qb < 2^31, qb <= 22 (the rounding trick's range)
-    int qb = 21, group = d.n_views;
-    const auto cap = [&](int bits) { return std::ldexp(1.0, 31 - bits) / w_view; };
-    if (cap(22) >= d.n_views) qb = 22;
-    else if (cap(21) >= d.n_views) qb = 21;
-    else {
-        qb = 21;
-        while (qb > 12 && cap(qb) < 1.0) --qb;
-        if (cap(qb) < 1.0) return;
-        group = (int)std::fmin((double)d.n_views, std::floor(cap(qb)));
-    }
+    int qb = 0, group = 0;
+    double w_view = 0;
+    if (!bt_fixed_point_plan(d, G->R, G->step, &qb, &group, &w_view)) return;
     G->bt_qb = qb; G->bt_group = group;
     const size_t n_acc = (size_t)(d.nx + G->bt_b) * (d.ny + G->bt_bs) * (d.nz + G->bt_bz);      // x-fastest, with margins
     const size_t n_acc_y = (size_t)(d.ny + G->bt_b) * (d.nx + G->bt_bs) * (d.nz + G->bt_bz);    // y-fastest

@@ -149,6 +149,7 @@ void plan_forward_tma(cbct_geometry *g);     // decides whether/how the TMA forw
 int launch_forward_tma(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
 void plan_backproject_tma(cbct_geometry *g); // after plan_forward_tma: same boxes, int32 accumulators
 void free_backproject_tma(cbct_geometry *g);
+bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int *qb, int *views_per_group, double *w_view);
 int launch_backproject_tma(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
 int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
 void free_bp_tables(cbct_geometry *g);

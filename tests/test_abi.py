@@ -64,6 +64,32 @@ def test_invalid_arguments_rejected_before_any_cuda_call():
     assert L.cbct_recon_create(ctypes.byref(binding.make_desc(G)[0]), 0, ctypes.byref(out)) == binding.CBCT_E_INVALID
 
 
+def test_backproject_fixed_point_plan_bounds_the_oracle_weight_sums():
+    """Host logic of the scatter backprojector: its int32 accumulators cannot wrap if the planned bound on the
+    sum of trilinear weights per voxel and view holds.  P^T of a one-view all-ones projection (oracle) IS that
+    sum times step, so the bound is checked against the oracle on ordinary and awkward geometries."""
+    from dataclasses import replace
+    from oracle import projector as op
+    G1 = syn.workload(1).geometry
+    cases = [G1, replace(G1, nu=24, nv=8, du=12.8, dv=12.8), replace(G1, step_mm=9.0), replace(G1, ox=30.0, oy=-20.0, oz=10.0),
+             syn.Geometry(24, 20, 40, 4.0, 4.0, 0.5, 28, 64, 5.0, 8.0, 1000.0, 1500.0, (0.2, 1.3, 2.9, 4.1, 5.6), oz=3.0,
+                          step_mm=0.4)]
+    for G in cases:
+        qb, group, w_view = binding.backproject_fixed_point_plan(G)
+        assert 12 <= qb <= 22 and 1 <= group <= G.n_views
+        assert group * w_view * 2.0 ** qb < 2.0 ** 31
+        for v in (0, G.n_views // 3, G.n_views - 1):
+            one = np.zeros(G.proj_shape)
+            one[v] = 1.0
+            measured = op.back_scatter(G, one).max() / G.step
+            assert measured <= w_view / 1.2, (G, v, measured, w_view)       # at least 20 % of margin left
+    # paper-size config: the whole 40 views need two groups at 21 bits (documented in DESIGN.md)
+    qb, group, w_view = binding.backproject_fixed_point_plan(syn.workload(4).geometry)
+    assert qb == 21 and group == 37
+    d, keep = binding.make_desc(replace(G1, sdd=900.0))
+    assert binding.lib().cbct_backproject_fixed_point_plan(ctypes.byref(d), None, None, None) == binding.CBCT_E_INVALID
+
+
 def test_no_cpu_fallback_without_a_device():
     """On a box without an sm_100 GPU the product path must refuse, not fall back."""
     import torch
