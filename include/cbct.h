@@ -100,6 +100,12 @@ int cbct_forward(const cbct_geometry *geom, const float *d_vol, float *d_proj, v
  * cbct_backproject_fixed_point_plan); otherwise voxel-driven in fp32 without atomics. */
 int cbct_backproject(const cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
 
+/* The paper's own backprojector, Eq. 3: f(x) = (dx dy dz)/(du dv) sum_theta L^3(u*)/(L0 l^2(x)) g(u*),
+ * g(u*) bilinear, zero outside the imager.  An APPROXIMATE adjoint of cbct_forward ("numerical error
+ * less than 1%"); provided for matched/unmatched comparisons, never used by cbct_cgls_*.
+ * Same buffers and conventions as cbct_backproject. */
+int cbct_backproject_eq3(const cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
+
 /* Host arithmetic only (no device needed): the fixed-point plan cbct_backproject uses for this geometry.
  *   max_weight_sum_per_view: upper bound on the sum of trilinear weights one voxel receives from one view;
  *   qb: contributions are rounded to multiples of max|g| / 2^qb;
