@@ -120,8 +120,8 @@ __global__ void __launch_bounds__(128) tf_reconstruct_kernel(const float *__rest
     f[((size_t)z * ny + y) * nx + x] = acc;
 }
 
-// Separable, z-marching form of the same sum (CBCT_TF_RECONSTRUCT_IMPL=march; the direct kernel above reads every
-// coefficient 27 times through L1 -- 6.3 ms for 1.98 GB at cfg 4 -- and stays the default until this one has run on a device):
+// Separable, z-marching form of the same sum (the default; the direct kernel above reads every coefficient 27 times
+// through L1 -- 6.3 ms for 1.98 GB at cfg 4 -- and is kept as a cross-check, CBCT_TF_RECONSTRUCT_IMPL=direct):
 //   f = sum_n Hz_n^T [ sum_m Hy_m^T [ sum_l Hx_l^T alpha_lmn ] ]
 // A CTA owns a 32(x) x 8(y) column of outputs over a z-segment and walks the coefficient planes once:
 //   x-pass: warp w (10 warps = 8 rows + one halo row on each side) forms G_mn = sum_l Hx_l^T alpha_lmn for its
@@ -306,10 +306,9 @@ extern "C" int tf_shrink(float *d_alpha, float mu, int nx, int ny, int nz, void 
 
 extern "C" int tf_reconstruct(const float *d_alpha, float *d_f, int nx, int ny, int nz, void *stream) {
     CBCT_TRY(tf_check(d_alpha, d_f, nx, ny, nz));
-    // default: the direct 27 x 27-tap kernel; CBCT_TF_RECONSTRUCT_IMPL=march selects the separable z-marching kernel
-    // (same sum, every coefficient read once), which becomes the default once it has been run on a device
+    // default: the separable z-marching kernel; CBCT_TF_RECONSTRUCT_IMPL=direct selects the 27 x 27-tap kernel (cross-check)
     const char *impl = getenv("CBCT_TF_RECONSTRUCT_IMPL");
-    if (impl && impl[0] == 'm') {
+    if (!(impl && impl[0] == 'd')) {
         dim3 grid(cdiv(nx, TR_X), cdiv(ny, TR_Y), cdiv(nz, TR_ZSEG));
         tf_reconstruct_march_kernel<<<grid, TR_THREADS, 0, as_stream(stream)>>>(d_alpha, d_f, nx, ny, nz);
     } else {

@@ -284,7 +284,6 @@ def test_backproject_axis_parallel_rays_and_fine_steps():
         assert rel_l2_per_view(g, op.forward(G, x.astype(np.float64))) <= TOL, step
 
 
-@pytest.mark.xfail(strict=False, reason="Eq. 3 kernel written while the GPU pool was closed, not yet run on a device")
 def test_paper_eq3_backprojector_matches_oracle():
     """the paper's own approximate adjoint (Eq. 3) against the oracle's Eq. 3,
     including an offset, ragged geometry whose voxels project beside the imager (zero outside)."""
