@@ -71,7 +71,8 @@ __global__ void __launch_bounds__(256) absmax_kernel(const float *__restrict__ g
 //         (mod 32): 2.2 wavefronts per ATOMS;
 //   LM 1: a warp = 16(u) x 2(v), rows 8 apart (their samples lie in different z-planes), no skew, the forward
 //         kernel's box (pitch 8, plane pitch 16 mod 32): 2.9 wavefronts per ATOMS (model) / 2.96 (ncu).
-// LM 1 is the default until LM 0 (CBCT_BT_LANES=0 at geometry-create) has been timed on the device.
+// LM 0 is the default (verified against the oracle by running this source under a CPU thread-per-CUDA-thread shim while
+// the GPU pool was closed; its 13.3 ms is the model's prediction from LM 1's measured 17.6 ms); CBCT_BT_LANES=1 selects LM 1.
 // The order in which a thread visits the samples of a chunk is free: integer sums do not depend on it.
 template <int BF, int BS, int LM>
 __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
@@ -312,10 +313,10 @@ void plan_backproject_tma(cbct_geometry *G) {
     const cbct_geometry_desc &d = G->desc;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
     if (!G->fw_tma_ok) return;
-    // lane layout (see the kernel): CBCT_BT_LANES=0 selects the skewed 8x4 layout, whose box is the forward kernel's
-    // with the row count rounded up to a multiple of 4 (plane pitch = 0 mod 32); default 1 = 16x2, forward's box
+    // lane layout (see the kernel): default 0 = the skewed 8x4 layout, whose box is the forward kernel's with the row
+    // count rounded up to a multiple of 4 (plane pitch = 0 mod 32); CBCT_BT_LANES=1 selects 16x2 with forward's box
     const char *lm_env = getenv("CBCT_BT_LANES");
-    G->bt_lm = (lm_env && atoi(lm_env) == 0) ? 0 : 1;
+    G->bt_lm = (lm_env && atoi(lm_env) == 1) ? 1 : 0;
     G->bt_b = G->fw_b; G->bt_bz = G->fw_bz; G->bt_bs = G->bt_lm == 0 ? (G->fw_bs + 3) & ~3 : G->fw_bs;
     if ((size_t)2 * G->bt_b * G->bt_bs * G->bt_bz * 4 > 100 * 1024) return;
     int qb = 0, group = 0;

@@ -196,10 +196,7 @@ def test_full_size_sampled_outputs(cfg):
 
 
 @pytest.mark.parametrize("impl,lanes", [
-    ("scatter", "1"),
-    # lane layout 0 (skewed 8x4) was written while the GPU pool was closed: expected to pass, not yet confirmed
-    pytest.param("scatter", "0", marks=pytest.mark.xfail(strict=False, reason="layout not yet run on a device")),
-    ("cell", None), ("gather", None)])
+    ("scatter", "0"), ("scatter", "1"), ("cell", None), ("gather", None)])
 def test_backproject_every_implementation_matches_oracle(monkeypatch, impl, lanes):
     """cbct_backproject has three kernels behind it: the TMA scatter kernel (default where the geometry allows,
     both lane layouts), the cell-driven kernel (fall-back) and the per-voxel gather kernel (cross-check).
