@@ -1,4 +1,5 @@
-"""ctypes front end of oracle/cbct_oracle.c (fp64 P, P^T, Eq. 3).  TEST INFRASTRUCTURE ONLY.
+"""ctypes front end of oracle/cbct_oracle.c (fp64 P, P^T, Eq. 3) and oracle/siddon_oracle.c (the paper's Siddon
+projector and its transpose).  TEST INFRASTRUCTURE ONLY.
 
 `geom` is any object with the attributes nx, ny, nz, dx, dy, dz, ox, oy, oz, nu, nv,
 du, dv, u0, v0, sad, sdd, angles (iterable of radians) and step (mm, > 0).
@@ -44,6 +45,12 @@ def lib():
         L.orc_back_eq3.argtypes = [gp, dp, dp]
         L.orc_sample_count.argtypes = [gp]
         L.orc_sample_count.restype = C.c_double
+        L.orc_siddon_forward.argtypes = [gp, dp, dp]
+        L.orc_siddon_back.argtypes = [gp, dp, dp]
+        L.orc_siddon_nnz.argtypes = [gp, C.c_long, C.c_long]
+        L.orc_siddon_nnz.restype = C.c_double
+        L.orc_siddon_forward.restype = None
+        L.orc_siddon_back.restype = None
         for fn in (L.orc_grid, L.orc_forward, L.orc_forward_rays, L.orc_back_scatter,
                    L.orc_back_gather, L.orc_back_gather_voxels, L.orc_back_eq3):
             fn.restype = None
@@ -144,3 +151,27 @@ def sample_count(geom):
     """Algorithmic sample count: sum over rays of chord(padded box)/step."""
     G, keep = _pack(geom)
     return float(lib().orc_sample_count(C.byref(G)))
+
+
+def siddon_forward(geom, f):
+    """g = P_siddon f: exact radiological path through piecewise-constant voxels (Siddon 1985)."""
+    G, keep = _pack(geom)
+    f = _vol(geom, f)
+    g = np.empty((G.n_views, geom.nv, geom.nu), dtype=np.float64)
+    lib().orc_siddon_forward(C.byref(G), _d(f), _d(g))
+    return g
+
+
+def siddon_back(geom, g):
+    """f = P_siddon^T g, literal ray-by-ray transpose."""
+    G, keep = _pack(geom)
+    g = _proj(geom, g)
+    f = np.empty((geom.nz, geom.ny, geom.nx), dtype=np.float64)
+    lib().orc_siddon_back(C.byref(G), _d(g), _d(f))
+    return f
+
+
+def siddon_nnz(geom, first=0, stride=1):
+    """Number of (ray, voxel) pairs with positive intersection length over rays first, first+stride, ..."""
+    G, keep = _pack(geom)
+    return float(lib().orc_siddon_nnz(C.byref(G), int(first), int(stride)))
