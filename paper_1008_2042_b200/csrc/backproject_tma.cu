@@ -30,23 +30,8 @@ namespace cbct {
 constexpr float BT_ROUND = 12582912.0f;          // 1.5 * 2^23: x + BT_ROUND holds round(x) in its low mantissa bits, |x| < 2^22
 constexpr int BT_ROUND_BITS = 0x4B400000;
 
-__device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap *map, int c0, int c1, int c2, unsigned src) {
-    asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
-                 "r"(src), "r"(c0), "r"(c1), "r"(c2)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
 // integer nearest to c = a*b (|c| < 2^22), in one FFMA + one IADD
 __device__ __forceinline__ int round_mul(float a, float b) { return __float_as_int(fmaf(a, b, BT_ROUND)) - BT_ROUND_BITS; }
-__device__ __forceinline__ void red_s32(unsigned addr, int v) { asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
-template <int OFF>
-__device__ __forceinline__ void red_s32_off(unsigned addr, int v) {
-    asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(v) : "memory");
-}
 
 // max |g| as the bit pattern of a non-negative float (orders like an unsigned integer); *out zeroed before
 __global__ void __launch_bounds__(256) absmax_kernel(const float *__restrict__ g, long long n, unsigned *out) {

@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
     if (tid == 0) {
         s_klo = 0x7fffffff; s_khi = -1;
         mbar_init(smem_u32(&bars[0]), 1); mbar_init(smem_u32(&bars[1]), 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_mbar_init();
     }
     if ((tu == 0 || tu == FT_TU - 1) && (tv == 0 || tv == FT_TV - 1)) corner[(tv ? 2 : 0) + (tu ? 1 : 0)] = rl;
     __syncthreads();
@@ -148,24 +148,16 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                         const unsigned a0 = base_r + 4u * idx;
                         float v000, v100, v010, v110, v001, v101, v011, v111;
                         if constexpr (BF > 0) {
-                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
-                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v100) : "r"(a0));
-                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v010) : "r"(a0), "n"(4 * BF));
-                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v110) : "r"(a0), "n"(4 * BF + 4));
-                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v001) : "r"(a0), "n"(4 * BF * BS));
-                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v101) : "r"(a0), "n"(4 * BF * BS + 4));
-                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v011) : "r"(a0), "n"(4 * BF * BS + 4 * BF));
-                            asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v111) : "r"(a0), "n"(4 * BF * BS + 4 * BF + 4));
+                            v000 = lds_f32_off<0>(a0);                    v100 = lds_f32_off<4>(a0);
+                            v010 = lds_f32_off<4 * BF>(a0);               v110 = lds_f32_off<4 * BF + 4>(a0);
+                            v001 = lds_f32_off<4 * BF * BS>(a0);          v101 = lds_f32_off<4 * BF * BS + 4>(a0);
+                            v011 = lds_f32_off<4 * BF * BS + 4 * BF>(a0); v111 = lds_f32_off<4 * BF * BS + 4 * BF + 4>(a0);
                         } else {
                             const unsigned a1 = a0 + 4u * pS, a2 = a0 + 4u * pZ, a3 = a2 + 4u * pS;
-                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v000) : "r"(a0));
-                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v100) : "r"(a0));
-                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v010) : "r"(a1));
-                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v110) : "r"(a1));
-                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v001) : "r"(a2));
-                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v101) : "r"(a2));
-                            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v011) : "r"(a3));
-                            asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v111) : "r"(a3));
+                            v000 = lds_f32(a0); v100 = lds_f32_off<4>(a0);
+                            v010 = lds_f32(a1); v110 = lds_f32_off<4>(a1);
+                            v001 = lds_f32(a2); v101 = lds_f32_off<4>(a2);
+                            v011 = lds_f32(a3); v111 = lds_f32_off<4>(a3);
                         }
                         const float a00 = fmaf(wf, v100 - v000, v000), a10 = fmaf(wf, v110 - v010, v010);
                         const float a01 = fmaf(wf, v101 - v001, v001), a11 = fmaf(wf, v111 - v011, v011);

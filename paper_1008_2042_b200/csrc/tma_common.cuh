@@ -1,11 +1,12 @@
 // tma_common.cuh -- pieces shared by the two TMA-staged projector kernels (forward_tma.cu: boxes of the volume are
 // LOADED into shared memory; backproject_tma.cu: boxes of accumulators are REDUCED back into global memory):
 // the pixel-tile / chunk planning (which voxel box covers samples k0..k0+kc-1 of a 16x16 pixel tile), mbarrier and
-// bulk-tensor PTX wrappers, and the tensor-map encoder.
+// the tensor-map encoder (the mbarrier / bulk-tensor PTX wrappers are in ptx.cuh).
 #pragma once
 #include <cuda.h>
 
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace cbct {
 
@@ -14,34 +15,6 @@ constexpr float FT_MAGIC = 8388608.0f;          // 2^23: x + 2^23 rounded down h
 constexpr unsigned FT_MAGIC_BITS = 0x4B000000u;
 
 struct RayL { float cf, cs, cz, bf, bs, bz; };  // ray in (fast, slow, z) index coordinates: P(tau) = c + b tau
-
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
-        : "memory");
-}
 
 struct Box3 { int lf, ls, lz; bool fits; };
 
