@@ -62,7 +62,12 @@ def lib():
     if not os.path.exists(LIB_PATH):
         raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1008_2042_b200.build` "
                           "(there is no CPU fallback)")
-    L = C.CDLL(LIB_PATH)
+    _lib = _declare(C.CDLL(LIB_PATH))
+    return _lib
+
+
+def _declare(L):
+    """argument / result types of every entry point of include/cbct.h on a loaded library"""
     vp, fp, ip = C.c_void_p, C.c_void_p, C.c_int
     L.cbct_status_string.restype = C.c_char_p
     L.cbct_status_string.argtypes = [ip]
@@ -102,7 +107,6 @@ def lib():
         if name != "cbct_status_string":
             getattr(L, name).restype = C.c_int
     L.cbct_launch_count.restype = C.c_longlong
-    _lib = L
     return L
 
 

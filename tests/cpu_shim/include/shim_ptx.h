@@ -1,0 +1,50 @@
+// tests/cpu_shim/include/shim_ptx.h -- TEST INFRASTRUCTURE, not product code.
+// Host emulation of the wrappers in paper_1008_2042_b200/csrc/ptx.cuh (same names, same signatures).  It is
+// force-included before the kernel sources and pre-defines ptx.cuh's include guard, so ptx.cuh contributes nothing.
+// Semantics follow the PTX ISA as used by the kernels: mbarrier phases with transaction counts, tiled 3-D bulk
+// tensor copies with zero fill of out-of-range elements, tensor reductions that skip them, bulk async-groups.
+// Hardware rules the emulation ENFORCES (a violation aborts the test with a message instead of faulting a GPU):
+// 128-byte aligned shared-memory box address, 16-byte aligned global address and strides, inner box extent a
+// multiple of 16 bytes, box extents <= 256, transaction bytes == box bytes, non-negative reduction coordinates,
+// shared addresses inside the launch's shared memory, no shared memory released under an unfinished bulk group.
+#pragma once
+#define CBCT_PTX_CUH_
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+namespace shim {
+void mbar_init(unsigned bar, unsigned count);
+void mbar_expect_tx(unsigned bar, unsigned bytes);
+void mbar_wait(unsigned bar, unsigned parity);
+void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar);
+void tma_reduce_add_3d(const CUtensorMap *map, int c0, int c1, int c2, unsigned src);
+void bulk_commit();
+void bulk_wait(int pending_allowed, bool read_only);
+}  // namespace shim
+
+namespace cbct {
+
+static inline unsigned smem_u32(const void *p) { return shim::cvta_shared(p); }
+static inline void mbar_init(unsigned bar, unsigned count) { shim::mbar_init(bar, count); }
+static inline void fence_mbar_init() {}
+static inline void mbar_expect_tx(unsigned bar, unsigned bytes) { shim::mbar_expect_tx(bar, bytes); }
+static inline void mbar_wait(unsigned bar, unsigned parity) { shim::mbar_wait(bar, parity); }
+static inline void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar) {
+    shim::tma_load_3d(dst, map, c0, c1, c2, bar);
+}
+static inline void tma_reduce_add_3d(const CUtensorMap *map, int c0, int c1, int c2, unsigned src) {
+    shim::tma_reduce_add_3d(map, c0, c1, c2, src);
+}
+static inline void bulk_commit() { shim::bulk_commit(); }
+static inline void bulk_wait_read0() { shim::bulk_wait(0, true); }
+static inline void bulk_wait0() { shim::bulk_wait(0, false); }
+static inline void fence_async_smem() {}
+
+static inline float lds_f32(unsigned addr) { return *static_cast<const float *>(shim::shared_ptr_of(addr, 4, "ld.shared.f32")); }
+template <int OFF>
+static inline float lds_f32_off(unsigned addr) { return lds_f32(addr + (unsigned)OFF); }
+static inline void red_s32(unsigned addr, int v) { *static_cast<int *>(shim::shared_ptr_of(addr, 4, "red.shared.add.s32")) += v; }
+template <int OFF>
+static inline void red_s32_off(unsigned addr, int v) { red_s32(addr + (unsigned)OFF, v); }
+
+}  // namespace cbct

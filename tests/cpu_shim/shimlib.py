@@ -1,0 +1,205 @@
+"""TEST INFRASTRUCTURE.  Loads tests/cpu_shim/build/libcbct_cpu_shim.so (the library's kernel sources compiled for the
+host, README.md) and offers the few calls the shim tests need.  Buffers handed to the library are guarded
+allocations of the shim (a read or write past the end is a segmentation fault, not a silent pass)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, HERE)
+import build as shim_build  # noqa: E402
+
+from paper_1008_2042_b200 import binding as cb  # noqa: E402  (GeometryDesc marshalling and the argtypes table only)
+
+_L = None
+
+
+def lib():
+    global _L
+    if _L is None:
+        L = cb._declare(C.CDLL(shim_build.build()))
+        L.shim_malloc.restype = C.c_void_p
+        L.shim_malloc.argtypes = [C.c_size_t]
+        L.shim_free.argtypes = [C.c_void_p]
+        L.shim_last_error.restype = C.c_char_p
+        L.shim_last_error.argtypes = []
+        L.shim_clear_error.argtypes = []
+        L.shim_kernel_log.restype = C.c_char_p
+        L.shim_kernel_log.argtypes = [C.c_int]
+        _L = L
+    return _L
+
+
+def kernel_log(clear: bool = True):
+    """names (with template arguments) of the kernels launched since the last call"""
+    return [ln.split(" grid=")[0] for ln in lib().shim_kernel_log(int(clear)).decode().splitlines()]
+
+
+class ShimViolation(AssertionError):
+    pass
+
+
+def check(status: int = 0, where: str = ""):
+    err = lib().shim_last_error().decode()
+    if err:
+        lib().shim_clear_error()
+        raise ShimViolation(f"{where}: {err}")
+    if status not in (0, 1):
+        raise RuntimeError(f"{where}: status {status} ({lib().cbct_status_string(status).decode()})")
+    return status
+
+
+class Buf:
+    """a guarded 'device' buffer"""
+
+    def __init__(self, shape, dtype=np.float32, init=None):
+        self.shape, self.dtype = tuple(shape), np.dtype(dtype)
+        self.nbytes = int(np.prod(self.shape)) * self.dtype.itemsize
+        self.ptr = lib().shim_malloc(max(self.nbytes, 1))
+        if init is not None:
+            a = np.ascontiguousarray(init, dtype=self.dtype)
+            assert a.shape == self.shape
+            C.memmove(self.ptr, a.ctypes.data, self.nbytes)
+
+    def numpy(self):
+        out = np.empty(self.shape, self.dtype)
+        C.memmove(out.ctypes.data, self.ptr, self.nbytes)
+        return out
+
+    def __del__(self):
+        if getattr(self, "ptr", None) and _L is not None:
+            _L.shim_free(self.ptr)
+            self.ptr = None
+
+
+def dev(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return Buf(a.shape, np.float32, a)
+
+
+class Geometry:
+    def __init__(self, geom):
+        self.spec = geom
+        d, self._keep = cb.make_desc(geom)
+        h = C.c_void_p()
+        check(lib().cbct_geometry_create(C.byref(d), C.byref(h)), "cbct_geometry_create")
+        self.handle = h
+        self.vol_shape = (geom.nz, geom.ny, geom.nx)
+        self.proj_shape = (len(tuple(geom.angles)), geom.nv, geom.nu)
+
+    def info(self):
+        nv, nr, K = C.c_int64(), C.c_int64(), C.c_int32()
+        t0, st, ns, ws = C.c_double(), C.c_double(), C.c_int64(), C.c_size_t()
+        check(lib().cbct_geometry_info(self.handle, C.byref(nv), C.byref(nr), C.byref(K), C.byref(t0), C.byref(st), C.byref(ns),
+                                       C.byref(ws)), "cbct_geometry_info")
+        return dict(n_vox=nv.value, n_rays=nr.value, K=K.value, t_min=t0.value, step=st.value, n_samples=ns.value)
+
+    def close(self):
+        if self.handle:
+            lib().cbct_geometry_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _call(self, name, src, out_shape):
+        a, out = dev(src), Buf(out_shape)
+        check(getattr(lib(), name)(self.handle, a.ptr, out.ptr, None), name)
+        return out.numpy()
+
+    def forward(self, f):
+        return self._call("cbct_forward", f, self.proj_shape)
+
+    def backproject(self, g):
+        return self._call("cbct_backproject", g, self.vol_shape)
+
+    def backproject_eq3(self, g):
+        return self._call("cbct_backproject_eq3", g, self.vol_shape)
+
+
+class Cgls:
+    def __init__(self, geometry: Geometry):
+        self.geometry = geometry
+        h = C.c_void_p()
+        check(lib().cbct_cgls_create(geometry.handle, C.byref(h)), "cbct_cgls_create")
+        self.handle = h
+
+    def __del__(self):
+        if getattr(self, "handle", None) and _L is not None:
+            _L.cbct_cgls_destroy(self.handle)
+            self.handle = None
+
+    def init(self, g, x, r, p):
+        check(lib().cbct_cgls_init(self.handle, g.ptr, x.ptr, r.ptr, p.ptr, None), "cbct_cgls_init")
+
+    def step(self, x, r, p):
+        check(lib().cbct_cgls_step(self.handle, x.ptr, r.ptr, p.ptr, None), "cbct_cgls_step")
+
+    def scalars(self, r=None):
+        out = (C.c_double * 5)()
+        s = check(lib().cbct_cgls_scalars(self.handle, r.ptr if r is not None else None, out, None), "cbct_cgls_scalars")
+        return dict(gamma=out[0], qq=out[1], alpha=out[2], beta=out[3], rr=out[4], breakdown=(s == 1))
+
+
+def _dims(shape):
+    nz, ny, nx = shape
+    return int(nx), int(ny), int(nz)
+
+
+def tf_decompose(f):
+    out = Buf((27,) + f.shape)
+    check(lib().tf_decompose(f.ptr, out.ptr, *_dims(f.shape), None), "tf_decompose")
+    return out
+
+
+def tf_shrink(alpha, mu):
+    check(lib().tf_shrink(alpha.ptr, float(mu), *_dims(alpha.shape[1:]), None), "tf_shrink")
+    return alpha
+
+
+def tf_reconstruct(alpha):
+    out = Buf(alpha.shape[1:])
+    check(lib().tf_reconstruct(alpha.ptr, out.ptr, *_dims(out.shape), None), "tf_reconstruct")
+    return out
+
+
+def tf_apply_fused(f, mu, clamp):
+    out = Buf(f.shape)
+    check(lib().tf_apply_fused(f.ptr, out.ptr, float(mu), int(bool(clamp)), *_dims(f.shape), None), "tf_apply_fused")
+    return out
+
+
+def mg_restrict(fine, fx=2, fy=2, fz=1):
+    nz, ny, nx = fine.shape
+    out = Buf((nz // fz, ny // fy, nx // fx))
+    check(lib().mg_restrict(fine.ptr, out.ptr, nx, ny, nz, fx, fy, fz, None), "mg_restrict")
+    return out
+
+
+def mg_prolong(coarse, fine_shape, fx=2, fy=2, fz=1):
+    nz, ny, nx = fine_shape
+    out = Buf(fine_shape)
+    check(lib().mg_prolong(coarse.ptr, out.ptr, nx, ny, nz, fx, fy, fz, None), "mg_prolong")
+    return out
+
+
+def a2_extrapolate(cur, prev, coef):
+    out = Buf(cur.shape)
+    check(lib().cbct_a2_extrapolate(cur.ptr, prev.ptr, out.ptr, float(coef), int(np.prod(cur.shape)), None), "cbct_a2_extrapolate")
+    return out
+
+
+def tf_reconstruct_volume(geom, g, n_levels, n_outer, n_cgls=3, mu=5e-4, momentum=True):
+    d, keep = cb.make_desc(geom)
+    arr = (C.c_int * n_levels)(*[int(v) for v in n_outer])
+    out = Buf((geom.nz, geom.ny, geom.nx))
+    check(lib().cbct_tf_reconstruct(C.byref(d), g.ptr, out.ptr, int(n_levels), arr, int(n_cgls), float(mu), int(bool(momentum)), None),
+          "cbct_tf_reconstruct")
+    return out

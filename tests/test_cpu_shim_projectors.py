@@ -1,0 +1,176 @@
+"""The projector KERNEL SOURCES executed on the host (tests/cpu_shim: one fiber per CUDA thread, guarded memory, TMA and
+mbarrier emulation with the hardware's rules enforced) against the fp64 oracle -- `-m "not gpu"`.
+
+This is not a parity claim (the `-m gpu` tests make that, on a B200, through the real library) and not a fallback
+(the package never loads the shim).  It checks, without a GPU, what a device would punish with an illegal-address
+fault, a hang or a wrong answer: indexing, box planning, alignment, barrier protocol, launch configuration.
+The cases mirror tests/test_gpu_projectors.py at the sizes the host can run in seconds; tolerances are the same.
+"""
+import math
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from cpu_shim import shimlib as sl
+from oracle import projector as op
+from paper_1008_2042_b200 import synthetic as syn
+
+TOL = 1e-5
+
+ODD = syn.Geometry(37, 29, 11, 2.0, 3.0, 5.0, 45, 19, 2.3, 3.1, 1000.0, 1500.0,
+                   (0.0, 0.4, math.pi / 4, math.pi / 2, 2.0, math.pi, 4.0, 5.5), ox=3.0, oy=-4.0, oz=2.0, u0=1.7, v0=-2.9,
+                   step_mm=0.7)
+# 4-divisible volume (the TMA kernels run), ragged detector (partial pixel tiles), offsets, all four view quadrants
+# plus the 45-degree tie of the orientation rule
+RAGGED_TMA = syn.Geometry(44, 36, 12, 2.0, 2.5, 4.0, 53, 27, 2.1, 2.9, 1000.0, 1500.0,
+                          (0.0, 0.3, math.pi / 4, 1.2, math.pi / 2, 2.2, 3 * math.pi / 4, math.pi, 3.9, 5.0, 5.9),
+                          ox=-3.0, oy=5.0, oz=1.5, u0=-2.2, v0=3.3, step_mm=0.9)
+
+
+def rel_l2_per_view(g, ref):
+    num = np.sqrt(np.sum((g.astype(np.float64) - ref) ** 2, axis=(1, 2)))
+    den = np.sqrt(np.sum(ref ** 2, axis=(1, 2)))
+    scale = np.max(np.abs(ref))
+    return np.max(np.where(den > 0, num / np.where(den > 0, den, 1.0), num / (scale if scale > 0 else 1.0)))
+
+
+def rel_l2(a, ref):
+    return float(np.linalg.norm(a.astype(np.float64).ravel() - ref.ravel()) / np.linalg.norm(ref.ravel()))
+
+
+def forward(G, f):
+    return sl.Geometry(G).forward(f)
+
+
+def back(G, y):
+    return sl.Geometry(G).backproject(y)
+
+
+@pytest.fixture(autouse=True)
+def _clean_log():
+    sl.kernel_log()
+    yield
+    sl.check(0, "end of test")
+
+
+@pytest.mark.parametrize("tma_mode", ["eager", "lazy"])
+def test_forward_tma_kernel(monkeypatch, tma_mode):
+    """eager: a TMA copy lands the moment it is issued (a missing 'buffer free' barrier corrupts the sums);
+    lazy: it lands when the mbarrier is first waited on (a missing wait reads poisoned memory)."""
+    monkeypatch.setenv("SHIM_TMA", tma_mode)
+    w, _, f0, _ = syn.make_inputs(1, noisy=False)
+    g = forward(w.geometry, f0)
+    assert any(k.startswith("cbct::forward_tma_kernel<") for k in sl.kernel_log())
+    assert rel_l2_per_view(g, op.forward(w.geometry, f0.astype(np.float64))) <= TOL
+    f = syn.uniform_volume(RAGGED_TMA, 71)
+    g = forward(RAGGED_TMA, f)
+    assert any(k.startswith("cbct::forward_tma_kernel<") for k in sl.kernel_log())
+    assert rel_l2_per_view(g, op.forward(RAGGED_TMA, f.astype(np.float64))) <= TOL
+
+
+def test_forward_fallback_kernels(monkeypatch):
+    f = syn.uniform_volume(ODD, 23)
+    ref = op.forward(ODD, f.astype(np.float64))
+    g = forward(ODD, f)                                   # nx, ny not divisible by 4: no tensor map
+    assert "cbct::forward_tiled_kernel" in sl.kernel_log()
+    assert rel_l2_per_view(g, ref) <= TOL
+    for impl in ("global", "tiled"):
+        monkeypatch.setenv("CBCT_FORWARD_IMPL", impl)
+        g = forward(ODD, f)
+        assert f"cbct::forward_{impl}_kernel" in sl.kernel_log()
+        assert rel_l2_per_view(g, ref) <= TOL, impl
+    monkeypatch.delenv("CBCT_FORWARD_IMPL")
+    for vox, pix in ((0.25, 3.0), (0.6, 2.0), (1.0, 1.2)):    # pixel tiles that do not fit the shared-memory box
+        G = syn.Geometry(96, 80, 24, vox, vox, 2 * vox, 40, 12, pix, pix, 1000.0, 1500.0, (0.1, 0.9, 2.4, 3.9),
+                         step_mm=0.8 * vox)
+        f = syn.uniform_volume(G, 24)
+        assert rel_l2_per_view(forward(G, f), op.forward(G, f.astype(np.float64))) <= TOL, (vox, pix)
+
+
+@pytest.mark.parametrize("lanes", ["0", "1"])
+@pytest.mark.parametrize("tma_mode", ["eager", "lazy"])
+def test_backproject_scatter_kernel(monkeypatch, lanes, tma_mode):
+    """both lane layouts of the TMA scatter kernel; signed input; lazy = tensor reductions read their shared-memory
+    box only at cp.async.bulk.wait_group (clearing the box too early loses the contributions)."""
+    monkeypatch.setenv("SHIM_TMA", tma_mode)
+    monkeypatch.setenv("CBCT_BT_LANES", lanes)
+    for G, seed in ((syn.workload(1).geometry, 34), (RAGGED_TMA, 72)):
+        y = syn.uniform_projections(G, seed) - 0.4
+        f = back(G, y)
+        assert any(k.startswith("cbct::backproject_scatter_kernel<") and k.endswith(f", {lanes}>") for k in sl.kernel_log())
+        assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, (lanes, tma_mode)
+
+
+@pytest.mark.parametrize("impl", ["cell", "gather"])
+def test_backproject_voxel_driven_kernels(monkeypatch, impl):
+    monkeypatch.setenv("CBCT_BACKPROJECT_IMPL", impl)
+    for G, seed in ((syn.workload(1).geometry, 34), (ODD, 25)):
+        y = syn.uniform_projections(G, seed) - 0.4
+        f = back(G, y)
+        assert any(k.startswith(f"cbct::backproject_{impl}_kernel") for k in sl.kernel_log())
+        assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, impl
+
+
+def test_backproject_default_dispatch_and_adjoint_identity():
+    G = syn.workload(1).geometry
+    x, y = syn.uniform_volume(G, 41), syn.uniform_projections(G, 41)
+    Px, PTy = forward(G, x), back(G, y)
+    log = sl.kernel_log()
+    assert any(k.startswith("cbct::backproject_scatter_kernel<") for k in log)      # the default where the geometry allows
+    lhs, rhs = float(np.sum(Px.astype(np.float64) * y)), float(np.sum(x.astype(np.float64) * PTy))
+    assert abs(lhs - rhs) <= TOL * abs(lhs)
+    y = syn.uniform_projections(ODD, 22) - 0.3                                     # no tensor map: the cell kernel
+    f = back(ODD, y)
+    assert any(k.startswith("cbct::backproject_cell_kernel<") for k in sl.kernel_log())
+    assert rel_l2(f, op.back_scatter(ODD, y.astype(np.float64))) <= TOL
+
+
+def test_backproject_scatter_fixed_point_properties():
+    G = syn.workload(1).geometry
+    y = syn.uniform_projections(G, 35)
+    f1, f2 = back(G, y), back(G, y)
+    assert np.array_equal(f1, f2)                                        # integer accumulation: order independent
+    assert np.array_equal(back(G, 4.0 * y), 4.0 * f1)                    # scaled by max|g|: exact for powers of two
+    y_hot = y.copy()
+    y_hot[3, G.nv // 2, G.nu // 3] = 100.0
+    assert rel_l2(back(G, y_hot), op.back_scatter(G, y_hot.astype(np.float64))) <= TOL
+    ones = np.ones(G.proj_shape, np.float32)                            # the weight sum the head-room plan bounds
+    f = back(G, ones)
+    assert rel_l2(f, op.back_scatter(G, ones.astype(np.float64))) <= TOL and np.all(f >= 0.0)
+
+
+def test_degenerate_inputs():
+    G = syn.workload(1).geometry
+    assert np.all(forward(G, np.zeros(G.vol_shape, np.float32)) == 0.0)
+    assert np.all(back(G, np.zeros(G.proj_shape, np.float32)) == 0.0)
+    Gm = replace(G, u0=5000.0)                                           # every ray misses the volume
+    assert np.all(forward(Gm, syn.uniform_volume(Gm, 1)) == 0.0)
+    assert np.all(back(Gm, syn.uniform_projections(Gm, 1)) == 0.0)
+    G1 = syn.Geometry(1, 1, 1, 4.0, 4.0, 4.0, 1, 1, 1.0, 1.0, 1000.0, 1500.0, (0.3,))
+    one = np.ones((1, 1, 1), np.float32)
+    g, ref = forward(G1, one), op.forward(G1, np.ones((1, 1, 1)))
+    assert abs(g[0, 0, 0] - ref[0, 0, 0]) <= TOL * ref[0, 0, 0]
+    f = back(G1, one)
+    assert abs(f[0, 0, 0] - op.back_scatter(G1, np.ones((1, 1, 1)))[0, 0, 0]) <= TOL * f[0, 0, 0]
+
+
+def test_steep_rays_axis_parallel_rays_and_odd_steps():
+    G = syn.Geometry(24, 20, 40, 4.0, 4.0, 0.5, 28, 64, 5.0, 8.0, 1000.0, 1500.0, (0.2, 1.3, 2.9, 4.1, 5.6),
+                     oz=3.0, step_mm=0.4)
+    y, x = syn.uniform_projections(G, 28) - 0.2, syn.uniform_volume(G, 29)
+    assert rel_l2(back(G, y), op.back_scatter(G, y.astype(np.float64))) <= TOL
+    assert rel_l2_per_view(forward(G, x), op.forward(G, x.astype(np.float64))) <= TOL
+    for step in (0.05, 0.9, 3.7):
+        G = syn.Geometry(20, 18, 7, 2.0, 2.0, 3.0, 21, 9, 2.5, 2.5, 1000.0, 1500.0, (0.0, math.pi / 2, math.pi, 1.0),
+                         step_mm=step)
+        y, x = syn.uniform_projections(G, 26), syn.uniform_volume(G, 27)
+        assert rel_l2(back(G, y), op.back_scatter(G, y.astype(np.float64))) <= TOL, step
+        assert rel_l2_per_view(forward(G, x), op.forward(G, x.astype(np.float64))) <= TOL, step
+
+
+def test_paper_eq3_backprojector_kernel():
+    for G, seed in ((syn.workload(1).geometry, 61), (ODD, 63)):
+        y = syn.uniform_projections(G, seed)
+        f = sl.Geometry(G).backproject_eq3(y)
+        assert rel_l2(f, op.back_eq3(G, y.astype(np.float64))) <= TOL

@@ -1,0 +1,128 @@
+"""CGLS vector kernels, the tight-frame kernels, multigrid transfers and the A2 driver executed on the host by
+tests/cpu_shim against the fp64 oracle -- `-m "not gpu"`.  Same purpose and caveats as test_cpu_shim_projectors.py:
+it checks the kernel sources for indexing / synchronisation mistakes without a GPU; parity is claimed by `-m gpu`.
+The cases mirror tests/test_gpu_solver.py (same tolerances) at host-sized inputs."""
+import numpy as np
+import pytest
+
+from cpu_shim import shimlib as sl
+from oracle import projector as op
+from oracle import solver as osv
+from paper_1008_2042_b200 import synthetic as syn
+
+
+def rel(a, ref):
+    return float(np.linalg.norm(np.asarray(a, np.float64).ravel() - ref.ravel()) / np.linalg.norm(ref.ravel()))
+
+
+def ops(G):
+    return (lambda x: op.forward(G, x)), (lambda r: op.back_scatter(G, r))
+
+
+@pytest.fixture(autouse=True)
+def _no_violation():
+    yield
+    sl.check(0, "end of test")
+
+
+def test_cgls_teacher_forced_step_scalars_and_breakdown():
+    w, _, f0, g = syn.make_inputs(1)
+    G = w.geometry
+    P, PT = ops(G)
+    h = sl.Geometry(G)
+    cg = sl.Cgls(h)
+    g64 = g.astype(np.float64)
+    d_g = sl.dev(g)
+    st_free = osv.cgls_init(P, PT, np.zeros(G.vol_shape), g64)
+    for step in range(2):
+        x32 = np.float32(st_free["x"])
+        st = osv.cgls_init(P, PT, x32.astype(np.float64), g64)
+        d_x, d_r, d_p = sl.dev(x32), sl.Buf(h.proj_shape), sl.Buf(h.vol_shape)
+        cg.init(d_g, d_x, d_r, d_p)
+        assert rel(d_r.numpy(), st["r"]) <= 1e-5 and rel(d_p.numpy(), st["p"]) <= 1e-5, step
+        sc = cg.scalars(d_r)
+        assert abs(sc["gamma"] - st["gamma"]) <= 2e-5 * st["gamma"]
+        st = osv.cgls_step(P, PT, st)
+        cg.step(d_x, d_r, d_p)
+        sc = cg.scalars(d_r)
+        assert not sc["breakdown"]
+        assert abs(sc["alpha"] - st["alpha"]) <= 2e-5 * abs(st["alpha"]) and abs(sc["beta"] - st["beta"]) <= 5e-5 * abs(st["beta"])
+        assert rel(d_x.numpy(), st["x"]) <= 1e-5 and rel(d_r.numpy(), st["r"]) <= 1e-5 and rel(d_p.numpy(), st["p"]) <= 1e-5
+        st_free = osv.cgls_step(P, PT, st_free)
+    zg, zx = sl.dev(np.zeros(h.proj_shape)), sl.dev(np.zeros(h.vol_shape))
+    d_r, d_p = sl.Buf(h.proj_shape), sl.Buf(h.vol_shape)
+    cg.init(zg, zx, d_r, d_p)
+    cg.step(zx, d_r, d_p)
+    sc = cg.scalars(d_r)
+    assert sc["breakdown"] and sc["alpha"] == 0.0 and np.all(zx.numpy() == 0) and np.all(np.isfinite(d_p.numpy()))
+
+
+SHAPES = [(16, 64, 64), (5, 7, 9), (1, 33, 40), (3, 1, 70), (9, 10, 1), (1, 1, 1), (6, 37, 131)]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_tf_three_call_path(shape):
+    rng = np.random.default_rng(sum(shape))
+    f = rng.standard_normal(shape).astype(np.float32)
+    a_ref = osv.tf_decompose(f.astype(np.float64))
+    d_f = sl.dev(f)
+    d_a = sl.tf_decompose(d_f)
+    a = d_a.numpy().astype(np.float64)
+    assert np.max(np.abs(a - a_ref)) <= 1e-5 * np.max(np.abs(a_ref))
+    sl.tf_shrink(d_a, 0.4)
+    assert np.max(np.abs(d_a.numpy() - osv.tf_shrink(a, 0.4))) <= 1e-5 * np.max(np.abs(a_ref))
+    r_ref = osv.tf_reconstruct(d_a.numpy().astype(np.float64))
+    assert np.max(np.abs(sl.tf_reconstruct(d_a).numpy() - r_ref)) <= 1e-5 * max(np.max(np.abs(r_ref)), 1e-30)
+    assert np.max(np.abs(sl.tf_reconstruct(sl.tf_decompose(d_f)).numpy() - f)) <= 1e-5 * np.max(np.abs(f))     # W^T W = I
+
+
+@pytest.mark.parametrize("impl", ["march", "direct"])
+@pytest.mark.parametrize("shape", SHAPES + [(31, 20, 45)])
+def test_tf_reconstruct_both_kernels(monkeypatch, shape, impl):
+    rng = np.random.default_rng(sum(shape) + 1)
+    a = rng.standard_normal((27,) + shape).astype(np.float32)
+    monkeypatch.setenv("CBCT_TF_RECONSTRUCT_IMPL", impl)
+    sl.kernel_log()
+    out = sl.tf_reconstruct(sl.dev(a)).numpy()
+    assert sl.kernel_log() == ["cbct::tf_reconstruct_march_kernel" if impl == "march" else "cbct::tf_reconstruct_kernel"]
+    r_ref = osv.tf_reconstruct(a.astype(np.float64))
+    assert np.max(np.abs(out - r_ref)) <= 1e-5 * np.max(np.abs(r_ref))
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("mu,clamp", [(0.0, False), (0.3, False), (0.3, True), (2.0, True), (1e6, False)])
+def test_tf_fused_matches_oracle(shape, mu, clamp):
+    rng = np.random.default_rng(sum(shape) + 1)
+    f = rng.standard_normal(shape).astype(np.float32)
+    ref = osv.tf_apply(f.astype(np.float64), mu, clamp_nonneg=clamp)
+    assert np.max(np.abs(sl.tf_apply_fused(sl.dev(f), mu, clamp).numpy() - ref)) <= 2e-5 * np.max(np.abs(f))
+
+
+@pytest.mark.parametrize("shape,fac", [((6, 8, 10), (2, 2, 1)), ((4, 6, 2), (2, 2, 2)), ((70, 64, 32), (2, 2, 1)),
+                                       ((3, 5, 8), (2, 1, 1)), ((2, 2, 2), (1, 1, 2))])
+def test_mg_restrict_prolong_and_extrapolate(shape, fac):
+    fx, fy, fz = fac
+    rng = np.random.default_rng(5)
+    fine = rng.random(shape).astype(np.float32)
+    cshape = (shape[0] // fz, shape[1] // fy, shape[2] // fx)
+    assert np.max(np.abs(sl.mg_restrict(sl.dev(fine), fx, fy, fz).numpy() - osv.mg_restrict(fine.astype(np.float64), fx, fy, fz))) <= 1e-6
+    coarse = rng.random(cshape).astype(np.float32)
+    assert np.max(np.abs(sl.mg_prolong(sl.dev(coarse), shape, fx, fy, fz).numpy() - osv.mg_prolong(coarse.astype(np.float64), fx, fy, fz))) <= 1e-6
+    b = rng.random(shape).astype(np.float32)
+    v = sl.a2_extrapolate(sl.dev(fine), sl.dev(b), 0.2817).numpy()
+    assert np.max(np.abs(v - (fine + 0.2817 * (fine.astype(np.float64) - b)))) <= 1e-6
+
+
+def test_multigrid_a2_driver_two_levels():
+    """the whole driver (cbct_tf_reconstruct: cascade, A2, CGLS, fused tight frame) on a small two-level problem"""
+    G = syn.Geometry(32, 32, 8, 4.0, 4.0, 4.0, 48, 16, 3.2, 3.2, 1000.0, 1500.0, tuple(2 * np.pi * k / 12 for k in range(12)))
+    f0 = syn.uniform_volume(G, 81)
+    g = op.forward(G, f0.astype(np.float64)).astype(np.float32)
+
+    def make_ops(fac):
+        return ops(G.coarsen_xy(fac) if fac > 1 else G)
+
+    mu, n_outer, n_cgls = 5e-4, [2, 2], 2
+    ref = osv.multigrid_a2(make_ops, G.vol_shape, g.astype(np.float64), 2, n_outer, n_cgls, mu)
+    out = sl.tf_reconstruct_volume(G, sl.dev(g), 2, n_outer, n_cgls, mu, True).numpy()
+    assert rel(out, ref) <= 1e-4
