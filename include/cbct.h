@@ -106,6 +106,21 @@ int cbct_backproject(const cbct_geometry *geom, const float *d_proj, float *d_vo
  * Same buffers and conventions as cbct_backproject. */
 int cbct_backproject_eq3(const cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
 
+/* The paper's OWN forward projector, PAPER.md:191 ("the line integral of Eq. (1) along an x-ray line using Siddon's
+ * ray-tracing algorithm"; also PAPER.md:211, :256), and its exact transpose:
+ *   g[ray] = sum over voxels |ray INTERSECT voxel| * f[voxel]   (lengths in mm),
+ * the volume being piecewise constant on the boxes [xb + ix dx, xb + (ix+1) dx] x ..., xb = ox - nx dx / 2, the ray the
+ * segment from the source to the pixel centre.  No sampling step: geom's step_mm is not used.  A second matched pair
+ * next to cbct_forward / cbct_backproject (which are the fixed-step trilinear pair north_star prescribes); CGLS in this
+ * library uses the trilinear pair.  Buffers and conventions as cbct_forward / cbct_backproject; outputs overwritten.
+ * The handle is not const: the first call allocates the pair's workspace (a y-fastest volume copy; for the transpose
+ * two int32 accumulator volumes) with cudaMalloc, i.e. the FIRST call synchronises the device; later calls are
+ * asynchronous on `stream`.  cbct_siddon_backproject accumulates in fixed point relative to max|g| (deterministic,
+ * error per contribution <= max|g| / 2^(qb+1) mm with qb >= 9 chosen from a bound on the path length one voxel can
+ * collect); CBCT_E_UNSUPPORTED if no qb satisfies the bound. */
+int cbct_siddon_forward(cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
+int cbct_siddon_backproject(cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
+
 /* Host arithmetic only (no device needed): the fixed-point plan cbct_backproject uses for this geometry.
  *   max_weight_sum_per_view: upper bound on the sum of trilinear weights one voxel receives from one view;
  *   qb: contributions are rounded to multiples of max|g| / 2^qb;

@@ -23,7 +23,7 @@ EXPORTS = [
     "cbct_profile_begin", "cbct_profile_end",
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
-    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3",
+    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_forward", "cbct_siddon_backproject",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
@@ -81,7 +81,8 @@ def _declare(L):
     L.cbct_geometry_info.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64),
                                      C.POINTER(C.c_size_t)]
-    for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host", "cbct_backproject_eq3"):
+    for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host", "cbct_backproject_eq3",
+                 "cbct_siddon_forward", "cbct_siddon_backproject"):
         getattr(L, name).argtypes = [vp, fp, fp, vp]
     L.cbct_backproject_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                                     C.POINTER(C.c_double)]
@@ -225,6 +226,18 @@ class Geometry:
         """The paper's approximate adjoint, Eq. 3 (not the transpose of forward)."""
         _check(lib().cbct_backproject_eq3(self.handle, _dptr(d_proj, self.n_rays), _dptr(d_vol, self.n_vox),
                                           _stream(stream)), "cbct_backproject_eq3")
+        return d_vol
+
+    def siddon_forward(self, d_vol, d_proj, stream=None):
+        """g = P_siddon f: the paper's own projector, exact path lengths through piecewise-constant voxels."""
+        _check(lib().cbct_siddon_forward(self.handle, _dptr(d_vol, self.n_vox), _dptr(d_proj, self.n_rays), _stream(stream)),
+               "cbct_siddon_forward")
+        return d_proj
+
+    def siddon_backproject(self, d_proj, d_vol, stream=None):
+        """f = P_siddon^T g, the exact transpose of siddon_forward."""
+        _check(lib().cbct_siddon_backproject(self.handle, _dptr(d_proj, self.n_rays), _dptr(d_vol, self.n_vox), _stream(stream)),
+               "cbct_siddon_backproject")
         return d_vol
 
     def forward_host(self, h_vol, h_proj, stream=None):

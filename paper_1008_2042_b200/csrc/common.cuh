@@ -129,6 +129,11 @@ struct cbct_geometry {
     unsigned *d_bt_absmax;
     alignas(64) unsigned char bt_map_x[128];
     alignas(64) unsigned char bt_map_y[128];
+    // Siddon pair (siddon.cu), allocated at the first call: y-fastest volume copy, two int32 accumulator volumes, max|g|
+    float *d_sd_volT;
+    int *d_sd_acc;
+    unsigned *d_sd_absmax;
+    int sd_qb, sd_group;
     size_t workspace_bytes;
 };
 
@@ -151,6 +156,13 @@ void plan_backproject_tma(cbct_geometry *g); // after plan_forward_tma: same box
 void free_backproject_tma(cbct_geometry *g);
 bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int *qb, int *views_per_group, double *w_view);
 int launch_backproject_tma(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
+void free_siddon(cbct_geometry *g);
+// kernels launched from more than one translation unit
+__global__ void transpose_vol_kernel(const float *__restrict__ v, float *__restrict__ vT, int nx, int ny);      // forward_tma.cu
+__global__ void absmax_kernel(const float *__restrict__ g, long long n, unsigned *out);                        // backproject_tma.cu
+__global__ void backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y, float *__restrict__ vol,
+                                            int nx, int ny, int pf, int ps, int pz, const unsigned *__restrict__ absmax_bits,
+                                            float step_over_two_qb, int accumulate);                             // backproject_tma.cu
 int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
 void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,

@@ -166,6 +166,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
     G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr; G->d_fw_volT = nullptr; G->fw_tma_ok = 0;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
+    G->d_sd_volT = nullptr; G->d_sd_acc = nullptr; G->d_sd_absmax = nullptr; G->sd_qb = 0; G->sd_group = 0;
     G->bp = BpTables{};
     G->workspace_bytes = 0;
 
@@ -237,6 +238,7 @@ extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     free_bp_tables(G);
     free_backproject_tma(G);
     cudaFree(G->d_fw_volT);
+    free_siddon(G);
     (void)cudaGetLastError();
     delete G;
     return CBCT_OK;

@@ -18,7 +18,9 @@ sys.path.insert(0, HERE)
 import cu2cpp  # noqa: E402
 
 # -mfma + contraction: a*b+c becomes one fused multiply-add, as nvcc's default -fmad=true does on the device
-CXXFLAGS = ["-std=c++17", "-O2", "-g", "-fPIC", "-fopenmp", "-mavx2", "-mfma", "-ffp-contract=fast", "-fno-strict-aliasing",
+# SHIM_CXX_EXTRA="-fsanitize=alignment,bounds -fno-sanitize-recover=all" adds UBSan's checks of vector-typed accesses and fixed arrays
+EXTRA = os.environ.get("SHIM_CXX_EXTRA", "").split()
+CXXFLAGS = EXTRA + ["-std=c++17", "-O2", "-g", "-fPIC", "-fopenmp", "-mavx2", "-mfma", "-ffp-contract=fast", "-fno-strict-aliasing",
             "-Wno-unknown-pragmas", "-Wno-attributes",
             "-I", os.path.join(HERE, "include"), "-I", CSRC, "-I", os.path.join(ROOT, "include"), "-include", "shim_ptx.h"]
 
@@ -57,7 +59,7 @@ def build(force: bool = False) -> str:
             bad = True
     if bad:
         raise RuntimeError("g++ failed on the CPU shim build")
-    subprocess.run(["g++", "-shared", "-fopenmp", "-o", LIB + ".tmp", *objs, "-ldl"], check=True)
+    subprocess.run(["g++", *EXTRA, "-shared", "-fopenmp", "-o", LIB + ".tmp", *objs, "-ldl"], check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB
 

@@ -123,6 +123,12 @@ class Geometry:
     def backproject_eq3(self, g):
         return self._call("cbct_backproject_eq3", g, self.vol_shape)
 
+    def siddon_forward(self, f):
+        return self._call("cbct_siddon_forward", f, self.proj_shape)
+
+    def siddon_backproject(self, g):
+        return self._call("cbct_siddon_backproject", g, self.vol_shape)
+
 
 class Cgls:
     def __init__(self, geometry: Geometry):

@@ -174,3 +174,44 @@ def test_paper_eq3_backprojector_kernel():
         y = syn.uniform_projections(G, seed)
         f = sl.Geometry(G).backproject_eq3(y)
         assert rel_l2(f, op.back_eq3(G, y.astype(np.float64))) <= TOL
+
+
+def test_siddon_pair_kernels():
+    """the paper's own projector (Siddon) and its transpose against the oracle's
+    sort-all-crossings definition; 4-divisible and ragged / offset geometries, axis-parallel rays (odd grid: the central
+    rays run through voxel centres, parallel to two axes), signed input."""
+    AXIS = syn.Geometry(21, 19, 7, 2.0, 2.0, 3.0, 21, 9, 2.5, 2.5, 1000.0, 1500.0, (0.0, math.pi / 2, math.pi, 1.0))
+    for G, seed in ((syn.workload(1).geometry, 91), (ODD, 92), (RAGGED_TMA, 93), (AXIS, 94)):
+        h = sl.Geometry(G)
+        x, y = syn.uniform_volume(G, seed), syn.uniform_projections(G, seed) - 0.3
+        g, f = h.siddon_forward(x), h.siddon_backproject(y)
+        assert {"cbct::siddon_forward_kernel", "cbct::siddon_scatter_kernel"} <= set(sl.kernel_log())
+        assert rel_l2_per_view(g, op.siddon_forward(G, x.astype(np.float64))) <= TOL
+        assert rel_l2(f, op.siddon_back(G, y.astype(np.float64))) <= TOL
+        lhs, rhs = float(np.sum(g.astype(np.float64) * y)), float(np.sum(x.astype(np.float64) * f))
+        assert abs(lhs - rhs) <= TOL * abs(lhs)
+        assert np.array_equal(f, h.siddon_backproject(y))                     # integer accumulation: reproducible
+    Gm = replace(syn.workload(1).geometry, u0=5000.0)                         # every ray misses the volume
+    hm = sl.Geometry(Gm)
+    assert np.all(hm.siddon_forward(syn.uniform_volume(Gm, 1)) == 0.0)
+    assert np.all(hm.siddon_backproject(syn.uniform_projections(Gm, 1)) == 0.0)
+
+
+def test_siddon_ray_inside_a_grid_plane_is_one_of_the_two_valid_answers():
+    """Even grid, centred odd detector: the central ray of the 0 / 90 / 180 degree views lies IN the grid plane y = 0
+    (x = 0), where 'the voxel the ray is in' has two equally valid answers (and in fp64 the 90-degree ray, whose
+    direction is 6e-17 off the plane, even switches sides at an arbitrary point).  What is unique is compared: every
+    other ray matches the oracle; the in-plane rays must lie between the oracle's answers for the volume shifted by
+    +-1e-6 mm across the plane (the two one-sided limits)."""
+    G = syn.Geometry(20, 18, 7, 2.0, 2.0, 3.0, 21, 9, 2.5, 2.5, 1000.0, 1500.0, (0.0, math.pi / 2, math.pi))
+    x = syn.uniform_volume(G, 95)
+    g = sl.Geometry(G).siddon_forward(x).astype(np.float64)
+    ref = op.siddon_forward(G, x.astype(np.float64))
+    lim = [op.siddon_forward(replace(G, ox=sx * 1e-6, oy=sy * 1e-6), x.astype(np.float64)) for sx in (-1, 1) for sy in (-1, 1)]
+    lo, hi = np.min(lim, axis=0), np.max(lim, axis=0)
+    in_plane = np.zeros(G.proj_shape, bool)
+    in_plane[:, :, G.nu // 2] = True                                           # u = 0: the column of rays inside the plane
+    assert np.linalg.norm((g - ref)[~in_plane]) <= TOL * np.linalg.norm(ref[~in_plane])
+    tol = 1e-5 * np.max(ref)
+    assert np.all(g[in_plane] >= lo[in_plane] - tol) and np.all(g[in_plane] <= hi[in_plane] + tol)
+    assert np.max(hi[in_plane] - lo[in_plane]) > 100 * tol                      # the case is not vacuous
