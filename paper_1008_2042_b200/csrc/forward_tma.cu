@@ -25,8 +25,11 @@ __device__ __forceinline__ float fetch0g(const float *__restrict__ vol, const De
     return __ldg(vol + ((size_t)iz * g.ny + iy) * g.nx + ix);
 }
 
-// BF, BS > 0: box pitches known at compile time (neighbour loads use immediate offsets); 0: run-time pitches
-template <int BF, int BS>
+// BF, BS > 0: box pitches known at compile time (neighbour loads use immediate offsets); 0: run-time pitches.
+// PK: the sample arithmetic on packed fp32 pairs (FFMA2 / FADD2, ptx.cuh): (F, S) positions, floors and fractions as one
+// pair, the lerp tree as pairs over z -- 3 FADD2 + 3 FFMA2 + 2 scalar instead of 14 scalar instructions.  Every lane is
+// the same IEEE operation in the same order as the scalar path, so both variants return bit-identical projections.
+template <int BF, int BS, bool PK>
 __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
                                                                  const float *__restrict__ vol, float *__restrict__ proj,
@@ -138,9 +141,35 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                     const float pSf = (float)pS, pZf = (float)pZ;
                     float part = 0.f, jf = 0.f;
                     const int n = jb - ja + 1;
+                    if constexpr (PK && BF > 0) {
+                        const f32x2 sFS = pack2(sF, sS), FS0 = pack2(F0, S0);
+                        const f32x2 magic2 = pack2(FT_MAGIC, FT_MAGIC), neg_magic2 = pack2(-FT_MAGIC, -FT_MAGIC);
 #pragma unroll 2
-                    for (int j = 0; j < n; ++j, jf += 1.f) {
-                        const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
+                        for (int j = 0; j < n; ++j, jf += 1.f) {
+                            const f32x2 FS = fma2(pack2(jf, jf), sFS, FS0);
+                            const float Z = fmaf(jf, sZ, Z0);
+                            const f32x2 rFS = add2(add2_rd(FS, magic2), neg_magic2);               // floors, exact
+                            const float rz = __fadd_rd(Z, FT_MAGIC) - FT_MAGIC;
+                            const f32x2 wFS = sub2(FS, rFS);
+                            const float wz = Z - rz;
+                            float rf, rs, wf, ws;
+                            unpack2(rFS, rf, rs); unpack2(wFS, wf, ws);
+                            const unsigned idx = (unsigned)__float2int_rn(fmaf(rz, pZf, fmaf(rs, pSf, rf)));
+                            const unsigned a0 = base_r + 4u * idx;
+                            // pairs over z: (lower plane, upper plane)
+                            const f32x2 p00 = pack2(lds_f32_off<0>(a0), lds_f32_off<4 * BF * BS>(a0));
+                            const f32x2 p10 = pack2(lds_f32_off<4>(a0), lds_f32_off<4 * BF * BS + 4>(a0));
+                            const f32x2 p01 = pack2(lds_f32_off<4 * BF>(a0), lds_f32_off<4 * BF * BS + 4 * BF>(a0));
+                            const f32x2 p11 = pack2(lds_f32_off<4 * BF + 4>(a0), lds_f32_off<4 * BF * BS + 4 * BF + 4>(a0));
+                            const f32x2 wf2 = pack2(wf, wf), ws2 = pack2(ws, ws);
+                            const f32x2 a0x = fma2(wf2, sub2(p10, p00), p00), a1x = fma2(wf2, sub2(p11, p01), p01);   // (a00, a01), (a10, a11)
+                            float b0, b1;
+                            unpack2(fma2(ws2, sub2(a1x, a0x), a0x), b0, b1);
+                            part += fmaf(wz, b1 - b0, b0);
+                        }
+                    } else {
+#pragma unroll 2
+                    for (int j = 0; j < n; ++j, jf += 1.f) {                        const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
                         const float qf = __fadd_rd(F, FT_MAGIC), qs = __fadd_rd(S, FT_MAGIC), qz = __fadd_rd(Z, FT_MAGIC);
                         const float rf = qf - FT_MAGIC, rs = qs - FT_MAGIC, rz = qz - FT_MAGIC;      // floors, exact
                         const float wf = F - rf, ws = S - rs, wz = Z - rz;
@@ -163,6 +192,7 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                         const float a01 = fmaf(wf, v101 - v001, v001), a11 = fmaf(wf, v111 - v011, v011);
                         const float b0 = fmaf(ws, a10 - a00, a00), b1 = fmaf(ws, a11 - a01, a01);
                         part += fmaf(wz, b1 - b0, b0);
+                    }
                     }
                     total += part;
                 }
@@ -211,15 +241,17 @@ __global__ void __launch_bounds__(256) transpose_vol_kernel(const float *__restr
 
 
 typedef void (*TmaKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, float *, float, int, int, int, int);
-static TmaKernel tma_kernel_ptr(int bf, int bs) {
-    if (bf == 24 && bs == 22) return forward_tma_kernel<24, 22>;
-    if (bf == 40 && bs == 30) return forward_tma_kernel<40, 30>;
-    if (bf == 40 && bs == 38) return forward_tma_kernel<40, 38>;
-    if (bf == 56 && bs == 46) return forward_tma_kernel<56, 46>;
-    if (bf == 56 && bs == 54) return forward_tma_kernel<56, 54>;
+// CBCT_FW_PACKED=0 selects the scalar instruction stream (same results); default: packed pairs
+static bool forward_packed() {
+    const char *e = getenv("CBCT_FW_PACKED");
+    return !(e && atoi(e) == 0);
+}
+static TmaKernel tma_kernel_ptr(int bf, int bs, bool pk) {
+#define CBCT_FK(F, S) if (bf == F && bs == S) return pk ? forward_tma_kernel<F, S, true> : forward_tma_kernel<F, S, false>;
+    CBCT_FK(24, 22) CBCT_FK(40, 30) CBCT_FK(40, 38) CBCT_FK(56, 46) CBCT_FK(56, 54)
+#undef CBCT_FK
     return nullptr;
 }
-static const void *tma_kernel_for(int bf, int bs) { return reinterpret_cast<const void *>(tma_kernel_ptr(bf, bs)); }
 
 // choose the box for this geometry (once, at create); fw_tma_ok = 0 when the TMA path cannot be used
 void plan_forward_tma(cbct_geometry *G) {
@@ -255,10 +287,12 @@ void plan_forward_tma(cbct_geometry *G) {
     CUtensorMap m;
     if (!make_map(&m, G->d_fw_volT, d.ny, d.nx, d.nz, bf, bs, bz)) return;
     std::memcpy(G->fw_map_y, &m, sizeof(m));
-    const void *kern = tma_kernel_for(bf, bs);
-    if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
-        (void)cudaGetLastError();
-        return;
+    for (int pk = 0; pk < 2; ++pk) {
+        const void *kern = reinterpret_cast<const void *>(tma_kernel_ptr(bf, bs, pk != 0));
+        if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return;
+        }
     }
     G->fw_tma_ok = 1;
 }
@@ -276,7 +310,7 @@ int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj
     }
     const size_t smem = (size_t)2 * ((G->fw_b * G->fw_bs * G->fw_bz + 31) & ~31) * 4;
     dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), g.n_views);
-    TmaKernel kern = tma_kernel_ptr(G->fw_b, G->fw_bs);
+    TmaKernel kern = tma_kernel_ptr(G->fw_b, G->fw_bs, forward_packed());
     if (!kern) return CBCT_E_UNSUPPORTED;
     kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz,
                                                        getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0);

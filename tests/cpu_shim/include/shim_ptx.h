@@ -47,4 +47,17 @@ static inline void red_s32(unsigned addr, int v) { *static_cast<int *>(shim::sha
 template <int OFF>
 static inline void red_s32_off(unsigned addr, int v) { red_s32(addr + (unsigned)OFF, v); }
 
+// packed fp32 pairs: two independent IEEE operations
+typedef unsigned long long f32x2;
+static inline f32x2 pack2(float lo, float hi) { f32x2 r; float v[2] = {lo, hi}; std::memcpy(&r, v, 8); return r; }
+static inline void unpack2(f32x2 p, float &lo, float &hi) { float v[2]; std::memcpy(v, &p, 8); lo = v[0]; hi = v[1]; }
+static inline f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    float a0, a1, b0, b1, c0, c1;
+    unpack2(a, a0, a1); unpack2(b, b0, b1); unpack2(c, c0, c1);
+    return pack2(std::fmaf(a0, b0, c0), std::fmaf(a1, b1, c1));
+}
+static inline f32x2 add2(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fadd_rn(a0, b0), __fadd_rn(a1, b1)); }
+static inline f32x2 sub2(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fadd_rn(a0, -b0), __fadd_rn(a1, -b1)); }
+static inline f32x2 add2_rd(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fadd_rd(a0, b0), __fadd_rd(a1, b1)); }
+
 }  // namespace cbct

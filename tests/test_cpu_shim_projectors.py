@@ -69,6 +69,19 @@ def test_forward_tma_kernel(monkeypatch, tma_mode):
     assert rel_l2_per_view(g, op.forward(RAGGED_TMA, f.astype(np.float64))) <= TOL
 
 
+def test_forward_tma_packed_and_scalar_streams_are_bit_identical(monkeypatch):
+    """forward_tma_kernel<.., PK>: the FFMA2 / FADD2 instruction stream (default) and the scalar one (CBCT_FW_PACKED=0)
+    perform the same IEEE operations in the same order."""
+    out = {}
+    for pk in ("1", "0"):
+        monkeypatch.setenv("CBCT_FW_PACKED", pk)
+        f = syn.uniform_volume(RAGGED_TMA, 73)
+        out[pk] = forward(RAGGED_TMA, f)
+        assert any(k.startswith("cbct::forward_tma_kernel<") and k.endswith("true>" if pk == "1" else "false>") for k in sl.kernel_log())
+    assert np.array_equal(out["0"], out["1"])
+    assert rel_l2_per_view(out["1"], op.forward(RAGGED_TMA, f.astype(np.float64))) <= TOL
+
+
 def test_forward_fallback_kernels(monkeypatch):
     f = syn.uniform_volume(ODD, 23)
     ref = op.forward(ODD, f.astype(np.float64))

@@ -75,6 +75,19 @@ def test_forward_matches_oracle_full(cfg):
     assert rel_l2_per_view(g, ref) <= TOL
 
 
+def test_forward_packed_and_scalar_instruction_streams_agree(monkeypatch):
+    """forward_tma_kernel has a packed-pair (FFMA2 / FADD2, default) and a scalar (CBCT_FW_PACKED=0) instruction stream;
+    both perform the same IEEE operations in the same order: bit-identical projections, both within the bar."""
+    w, _, f0, _ = syn.make_inputs(2, noisy=False)
+    ref = op.forward(w.geometry, f0.astype(np.float64))
+    out = {}
+    for pk in ("1", "0"):
+        monkeypatch.setenv("CBCT_FW_PACKED", pk)
+        out[pk], _ = gpu_forward(w.geometry, f0)
+        assert rel_l2_per_view(out[pk], ref) <= TOL, pk
+    assert np.array_equal(out["0"], out["1"])
+
+
 def test_forward_ragged_offset_geometry():
     f = syn.uniform_volume(ODD, 21)
     g, _ = gpu_forward(ODD, f)
