@@ -20,6 +20,7 @@ void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, u
 void tma_reduce_add_3d(const CUtensorMap *map, int c0, int c1, int c2, unsigned src);
 void bulk_commit();
 void bulk_wait(int pending_allowed, bool read_only);
+void bank_record(unsigned addr, unsigned kind);       // kind 0: ld.shared, 1: red.shared (bank statistics, off by default)
 }  // namespace shim
 
 namespace cbct {
@@ -40,10 +41,10 @@ static inline void bulk_wait_read0() { shim::bulk_wait(0, true); }
 static inline void bulk_wait0() { shim::bulk_wait(0, false); }
 static inline void fence_async_smem() {}
 
-static inline float lds_f32(unsigned addr) { return *static_cast<const float *>(shim::shared_ptr_of(addr, 4, "ld.shared.f32")); }
+static inline float lds_f32(unsigned addr) { shim::bank_record(addr, 0); return *static_cast<const float *>(shim::shared_ptr_of(addr, 4, "ld.shared.f32")); }
 template <int OFF>
 static inline float lds_f32_off(unsigned addr) { return lds_f32(addr + (unsigned)OFF); }
-static inline void red_s32(unsigned addr, int v) { *static_cast<int *>(shim::shared_ptr_of(addr, 4, "red.shared.add.s32")) += v; }
+static inline void red_s32(unsigned addr, int v) { shim::bank_record(addr, 1); *static_cast<int *>(shim::shared_ptr_of(addr, 4, "red.shared.add.s32")) += v; }
 template <int OFF>
 static inline void red_s32_off(unsigned addr, int v) { red_s32(addr + (unsigned)OFF, v); }
 

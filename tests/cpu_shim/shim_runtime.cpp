@@ -18,6 +18,7 @@
 #include <ucontext.h>
 #include <unistd.h>
 
+#include <algorithm>
 #include <map>
 #include <mutex>
 #include <string>
@@ -120,10 +121,12 @@ struct Fiber {
     uint3 tid;
     int lin;
     unsigned wmask; WarpOp wop; uint64_t wpayload, wresult; int warg;
+    unsigned seq;                                     // ordinal of the next shared-memory instruction since the last barrier
     std::vector<BulkOp> open_group;                   // tensor reductions issued since the last commit
     std::vector<std::vector<BulkOp>> groups;          // committed, not yet executed (lazy mode), oldest first
 };
 struct PendingLoad { CUtensorMap map; int c[3]; unsigned dst, bar; };
+struct BankRec { unsigned warp, seq, addr, kind; };     // one lane of one shared-memory instruction (bank statistics)
 struct StaticShared { const void *key; unsigned char *ptr; size_t bytes; unsigned vaddr; };
 struct Worker {
     std::vector<Fiber> fibers;
@@ -138,6 +141,8 @@ struct Worker {
     std::vector<StaticShared> statics;
     unsigned static_next = 0x100;
     std::vector<PendingLoad> loads;                   // lazy mode: issued, not yet performed
+    std::vector<BankRec> bank;                        // bank statistics of the running block
+    unsigned epoch = 0;                               // __syncthreads count: re-aligns the lanes' instruction ordinals
 };
 static thread_local Worker *tw = nullptr;
 static const size_t STACK_BYTES = 256 * 1024, DYN_MAX = 232448;       // 227 KiB
@@ -238,6 +243,46 @@ unsigned cvta_shared(const void *p) {
     fail("__cvta_generic_to_shared: %p is not in this block's shared memory", p);
 }
 
+// ---- shared-memory bank statistics (shim_bank_stats_enable) ----------------------------------------------------------------------
+// A warp's lanes execute the k-th ld.shared / red.shared after a barrier together (lanes that have run out of loop
+// iterations are masked off), so grouping the recorded lane addresses by (warp, barrier epoch, ordinal) reconstructs the
+// warp instructions.  Wavefronts of one instruction = the largest number of requests falling on one of the 32 banks:
+// for loads, lanes reading the same word share a request (broadcast); for atomic reductions every lane is a request
+// (measured on B200: 32 clk when all lanes hit one word, profiles/README.md).
+static bool g_bank_on = false;
+static std::mutex g_bank_mu;
+static double g_bank_tot[4] = {0, 0, 0, 0};             // ld instr, ld wavefronts, red instr, red wavefronts
+void bank_record(unsigned addr, unsigned kind) {
+    if (!g_bank_on) return;
+    Worker *w = tw;
+    Fiber &f = w->fibers[w->cur];
+    w->bank.push_back(BankRec{(unsigned)f.lin >> 5, (w->epoch << 18) | (f.seq++ & 0x3ffff), addr, kind});
+}
+static void bank_flush(Worker *w) {
+    if (w->bank.empty()) return;
+    std::sort(w->bank.begin(), w->bank.end(), [](const BankRec &a, const BankRec &b) {
+        return a.warp != b.warp ? a.warp < b.warp : (a.seq != b.seq ? a.seq < b.seq : a.addr < b.addr);
+    });
+    double tot[4] = {0, 0, 0, 0};
+    for (size_t i = 0; i < w->bank.size();) {
+        size_t j = i;
+        int per_bank[32] = {0};
+        unsigned last_word[32];
+        for (; j < w->bank.size() && w->bank[j].warp == w->bank[i].warp && w->bank[j].seq == w->bank[i].seq; ++j) {
+            const unsigned word = w->bank[j].addr >> 2, b = word & 31;
+            if (w->bank[i].kind == 0 && per_bank[b] && last_word[b] == word) continue;       // broadcast (sorted by address)
+            ++per_bank[b]; last_word[b] = word;
+        }
+        int wf = 0;
+        for (int b = 0; b < 32; ++b) wf = std::max(wf, per_bank[b]);
+        tot[2 * w->bank[i].kind] += 1; tot[2 * w->bank[i].kind + 1] += wf;
+        i = j;
+    }
+    w->bank.clear();
+    std::lock_guard<std::mutex> lk(g_bank_mu);
+    for (int k = 0; k < 4; ++k) g_bank_tot[k] += tot[k];
+}
+
 void *shared_ptr_of(unsigned addr, size_t bytes, const char *what) {
     Worker *w = tw;
     if (addr >= DYN_VADDR) {
@@ -324,6 +369,7 @@ static void complete_warp(Worker *w, int warp) {
 static std::mutex g_attr_mu;
 static std::unordered_map<const void *, int> g_max_dyn;
 static std::string g_cur_kernel;
+static long long g_block_stride = 1;                   // statistics runs: execute every n-th block only (outputs incomplete)
 static std::string g_kernel_log;                       // demangled names of the kernels launched, one per line
 
 static void log_kernel(const void *func, dim3 grid, dim3 block, size_t smem) {
@@ -355,11 +401,12 @@ static void run_block(Worker *w, const std::function<void()> &body, dim3 grid, d
     w->dyn_base = w->dyn_region + DYN_MAX - ((smem + 127) & ~(size_t)127);
     if (smem) std::memset(w->dyn_base, 0xFF, smem);
     w->loads.clear();
+    w->bank.clear(); w->epoch = 0;
     if ((int)w->fibers.size() < n) w->fibers.resize(n);
     gridDim = grid; blockDim = block; blockIdx = bid;
     for (int i = 0; i < n; ++i) {
         Fiber &f = w->fibers[i];
-        f.state = READY; f.lin = i;
+        f.state = READY; f.lin = i; f.seq = 0;
         f.tid = uint3{(unsigned)i % block.x, ((unsigned)i / block.x) % block.y, (unsigned)i / (block.x * block.y)};
         f.open_group.clear(); f.groups.clear();
         getcontext(&f.ctx);
@@ -389,7 +436,8 @@ static void run_block(Worker *w, const std::function<void()> &body, dim3 grid, d
         for (int i = 0; i < n; ++i) waiting += w->fibers[i].state == WAIT_BLOCK;
         if (waiting && waiting == w->live) {
             for (int i = 0; i < n; ++i)
-                if (w->fibers[i].state == WAIT_BLOCK) w->fibers[i].state = READY;
+                if (w->fibers[i].state == WAIT_BLOCK) { w->fibers[i].state = READY; w->fibers[i].seq = 0; }
+            ++w->epoch;
             w->progress = true;
         }
         idle_passes = w->progress ? 0 : idle_passes + 1;
@@ -404,6 +452,7 @@ static void run_block(Worker *w, const std::function<void()> &body, dim3 grid, d
         }
     }
     if (!w->loads.empty() && !w->aborted && !g_failed) record_error("block ends with a TMA load in flight that nobody waited for");
+    bank_flush(w);
 }
 
 void launch(const void *func, dim3 grid, dim3 block, size_t smem, const std::function<void()> &body) {
@@ -433,7 +482,7 @@ void launch(const void *func, dim3 grid, dim3 block, size_t smem, const std::fun
         Worker *w = acquire_worker();
 #pragma omp for schedule(dynamic, 1)
         for (long long b = 0; b < nblocks; ++b) {
-            if (g_failed) continue;
+            if (g_failed || (g_block_stride > 1 && b % g_block_stride)) continue;
             const uint3 bid{(unsigned)(b % grid.x), (unsigned)((b / grid.x) % grid.y), (unsigned)(b / ((long long)grid.x * grid.y))};
             run_block(w, body, grid, block, bid, smem);
         }
@@ -621,6 +670,16 @@ const char *shim_kernel_log(int clear) {               // what was launched sinc
     copy = shim::g_kernel_log;
     if (clear) shim::g_kernel_log.clear();
     return copy.c_str();
+}
+void shim_bank_stats_enable(int on, long long block_stride) {   // block_stride > 1: run every n-th block only (statistics, not results)
+    shim::g_bank_on = on != 0;
+    shim::g_block_stride = block_stride > 1 ? block_stride : 1;
+    std::lock_guard<std::mutex> lk(shim::g_bank_mu);
+    for (double &v : shim::g_bank_tot) v = 0;
+}
+void shim_bank_stats(double out[4]) {                   // {ld.shared instr, wavefronts, red.shared instr, wavefronts} per warp
+    std::lock_guard<std::mutex> lk(shim::g_bank_mu);
+    for (int k = 0; k < 4; ++k) out[k] = shim::g_bank_tot[k];
 }
 void shim_clear_error(void) {
     std::lock_guard<std::mutex> lk(shim::g_err_mu);

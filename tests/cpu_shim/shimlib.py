@@ -28,6 +28,8 @@ def lib():
         L.shim_last_error.restype = C.c_char_p
         L.shim_last_error.argtypes = []
         L.shim_clear_error.argtypes = []
+        L.shim_bank_stats_enable.argtypes = [C.c_int, C.c_longlong]
+        L.shim_bank_stats.argtypes = [C.POINTER(C.c_double)]
         L.shim_kernel_log.restype = C.c_char_p
         L.shim_kernel_log.argtypes = [C.c_int]
         _L = L
@@ -37,6 +39,27 @@ def lib():
 def kernel_log(clear: bool = True):
     """names (with template arguments) of the kernels launched since the last call"""
     return [ln.split(" grid=")[0] for ln in lib().shim_kernel_log(int(clear)).decode().splitlines()]
+
+
+class bank_stats:
+    """with bank_stats(block_stride) as st: ... ; st.ld / st.red = shared-memory wavefronts per warp instruction.
+    block_stride > 1 executes only every n-th block of each launch: statistics only, the outputs are incomplete."""
+
+    def __init__(self, block_stride: int = 1):
+        self.stride = block_stride
+
+    def __enter__(self):
+        lib().shim_bank_stats_enable(1, self.stride)
+        return self
+
+    def __exit__(self, *exc):
+        out = (C.c_double * 4)()
+        lib().shim_bank_stats(out)
+        lib().shim_bank_stats_enable(0, 1)
+        self.ld_instr, self.ld_wavefronts, self.red_instr, self.red_wavefronts = out[0], out[1], out[2], out[3]
+        self.ld = out[1] / out[0] if out[0] else float("nan")
+        self.red = out[3] / out[2] if out[2] else float("nan")
+        return False
 
 
 class ShimViolation(AssertionError):

@@ -228,3 +228,27 @@ def test_siddon_ray_inside_a_grid_plane_is_one_of_the_two_valid_answers():
     tol = 1e-5 * np.max(ref)
     assert np.all(g[in_plane] >= lo[in_plane] - tol) and np.all(g[in_plane] <= hi[in_plane] + tol)
     assert np.max(hi[in_plane] - lo[in_plane]) > 100 * tol                      # the case is not vacuous
+
+
+def test_shared_memory_bank_model_reproduces_ncu_and_ranks_the_lane_layouts(monkeypatch):
+    """The shim groups the lanes' shared-memory addresses into warp instructions and counts wavefronts (README.md).
+    At the paper-size geometry, on a sample of CTAs: the 16x2 lane layout of the scatter kernel must reproduce what
+    ncu measured on a B200 (profiles/README.md: 5.03e9 shared wavefronts / 1.63e9 ATOMS = 2.96 per instruction, the
+    kernel's bound), which pins the model; the skewed 8x4 layout that is now the default must be clearly below it; the
+    forward kernel's loads must be nearly conflict-free (ncu: 1.93e9 wavefronts for 1.67e9 LDS + staging)."""
+    G = syn.workload(4).geometry
+    y, x = syn.uniform_projections(G, 1), syn.uniform_volume(G, 1)
+    stride = 311                                                   # 99 of the 30720 CTAs of a launch, spread over views and tiles
+    red = {}
+    for lanes in ("1", "0"):
+        monkeypatch.setenv("CBCT_BT_LANES", lanes)
+        h = sl.Geometry(G)
+        with sl.bank_stats(stride) as st:
+            h.backproject(y)
+        red[lanes] = st.red
+    assert abs(red["1"] - 2.96) <= 0.15, red                       # model vs ncu
+    assert red["0"] <= 2.40 and red["0"] <= 0.82 * red["1"], red   # the default layout: about a quarter fewer wavefronts
+    h = sl.Geometry(G)
+    with sl.bank_stats(stride) as st:
+        h.forward(x)
+    assert st.ld <= 1.15, st.ld
