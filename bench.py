@@ -194,10 +194,16 @@ def main():
             e[2].record(); cb.tf_apply_fused(d_vol, d_out, MU, True)
             e[3].record()
             evs.append(e)
+        s = [torch.cuda.Event(enable_timing=True) for _ in range(3)]     # the paper's own pair (Siddon), warm then timed
+        geom.siddon_forward(d_vol, d_proj); geom.siddon_backproject(d_g, d_out)
+        s[0].record(); geom.siddon_forward(d_vol, d_proj)
+        s[1].record(); geom.siddon_backproject(d_g, d_out)
+        s[2].record()
         torch.cuda.synchronize()
         e = evs[-1]
         print(json.dumps(dict(kernels_only=True, workload=args.workload, p_ms=e[0].elapsed_time(e[1]),
                               pt_ms=e[1].elapsed_time(e[2]), tf_fused_ms=e[2].elapsed_time(e[3]),
+                              siddon_p_ms=s[0].elapsed_time(s[1]), siddon_pt_ms=s[1].elapsed_time(s[2]),
                               samples=geom.n_samples)), flush=True)
         return
 
@@ -278,6 +284,14 @@ def main():
     ms_p = float(np.median(timed(lambda: geom.forward(d_vol, d_proj), 5)))
     ms_pt = float(np.median(timed(lambda: geom.backproject(d_g, d_tmp), 5)))
     ms_tf = float(np.median(timed(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True), 5)))
+    # the paper's own pair (Siddon) and the scalar instruction stream of P: context numbers
+    geom.siddon_forward(d_vol, d_proj); geom.siddon_backproject(d_g, d_tmp)
+    ms_sp = float(np.median(timed(lambda: geom.siddon_forward(d_vol, d_proj), 3)))
+    ms_spt = float(np.median(timed(lambda: geom.siddon_backproject(d_g, d_tmp), 3)))
+    os.environ["CBCT_FW_PACKED"] = "0"
+    geom.forward(d_vol, d_proj)
+    ms_p_scalar = float(np.median(timed(lambda: geom.forward(d_vol, d_proj), 5)))
+    del os.environ["CBCT_FW_PACKED"]
 
     # ---- the paper's full reconstruction, end to end (context number; 3 levels, 5/10/15) ----
     full_recon_s = None
@@ -344,7 +358,8 @@ def main():
                  d2h_bytes_per_step=int(h_f.numel() * 4), ms_per_step=e2e_ms / args.steps,
                  api="cbct_recon_run_host (HOST g in, HOST f out) + TF/MG tail on the returned volume"),
         roofline=roofline, cpu_baseline=cpu_baseline,
-        extra=dict(p_ms=ms_p, pt_ms=ms_pt, tf_fused_ms=ms_tf,
+        extra=dict(p_ms=ms_p, pt_ms=ms_pt, tf_fused_ms=ms_tf, p_scalar_stream_ms=ms_p_scalar,
+                   siddon_p_ms=ms_sp, siddon_pt_ms=ms_spt,
                    p_gsamples_s=geom.n_samples / ms_p / 1e6, pt_gsamples_s=geom.n_samples / ms_pt / 1e6,
                    s_per_cgls_iter=(ms_p + ms_pt) * 1e-3 + 0.0,
                    s_per_cgls_iter_in_step=(ms_f / max(n_f, 1) + ms_b / max(n_b, 1)) * 1e-3,
