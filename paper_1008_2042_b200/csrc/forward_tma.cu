@@ -26,9 +26,9 @@ __device__ __forceinline__ float fetch0g(const float *__restrict__ vol, const De
 }
 
 // BF, BS > 0: box pitches known at compile time (neighbour loads use immediate offsets); 0: run-time pitches.
-// PK: the sample arithmetic on packed fp32 pairs (FFMA2 / FADD2, ptx.cuh): (F, S) positions, floors and fractions as one
-// pair, the lerp tree as pairs over z -- 3 FADD2 + 3 FFMA2 + 2 scalar instead of 14 scalar instructions.  Every lane is
-// the same IEEE operation in the same order as the scalar path, so both variants return bit-identical projections.
+// PK: the sample arithmetic on packed fp32 pairs (FFMA2 / FADD2, ptx.cuh), two consecutive samples of the ray per pair:
+// positions, floors, fractions, element index and the seven lerps are all pair instructions.  Every lane is the same IEEE
+// operation in the same order as the scalar path, so both variants return bit-identical projections.
 template <int BF, int BS, bool PK>
 __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
@@ -142,34 +142,67 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                     float part = 0.f, jf = 0.f;
                     const int n = jb - ja + 1;
                     if constexpr (PK && BF > 0) {
-                        const f32x2 sFS = pack2(sF, sS), FS0 = pack2(F0, S0);
+                        // Two samples (j, j+1) per iteration, one in each lane of a pair: positions, floors, fractions, the
+                        // element index and all seven lerps are pair instructions.  The two contributions are added to `part`
+                        // one after the other, so the sum is formed in the scalar stream's order.
+                        const f32x2 sF2 = pack2(sF, sF), sS2 = pack2(sS, sS), sZ2 = pack2(sZ, sZ);
+                        const f32x2 F02 = pack2(F0, F0), S02 = pack2(S0, S0), Z02 = pack2(Z0, Z0);
                         const f32x2 magic2 = pack2(FT_MAGIC, FT_MAGIC), neg_magic2 = pack2(-FT_MAGIC, -FT_MAGIC);
-#pragma unroll 2
-                        for (int j = 0; j < n; ++j, jf += 1.f) {
-                            const f32x2 FS = fma2(pack2(jf, jf), sFS, FS0);
+                        const f32x2 pS2 = pack2(pSf, pSf), pZ2 = pack2(pZf, pZf), two2 = pack2(2.f, 2.f);
+                        f32x2 jj = pack2(0.f, 1.f);
+                        int j = 0;
+#pragma unroll 1
+                        for (; j + 1 < n; j += 2, jj = add2(jj, two2)) {
+                            const f32x2 F = fma2(jj, sF2, F02), S = fma2(jj, sS2, S02), Z = fma2(jj, sZ2, Z02);
+                            const f32x2 rF = add2(add2_rd(F, magic2), neg_magic2), rS = add2(add2_rd(S, magic2), neg_magic2),
+                                        rZ = add2(add2_rd(Z, magic2), neg_magic2);                 // floors, exact
+                            const f32x2 wF = sub2(F, rF), wS = sub2(S, rS), wZ = sub2(Z, rZ);
+                            float ia, ib;
+                            unpack2(fma2(rZ, pZ2, fma2(rS, pS2, rF)), ia, ib);
+                            const unsigned aA = base_r + 4u * (unsigned)__float2int_rn(ia), aB = base_r + 4u * (unsigned)__float2int_rn(ib);
+                            // pairs over the two samples
+                            const f32x2 v000 = pack2(lds_f32_off<0>(aA), lds_f32_off<0>(aB));
+                            const f32x2 v100 = pack2(lds_f32_off<4>(aA), lds_f32_off<4>(aB));
+                            const f32x2 v010 = pack2(lds_f32_off<4 * BF>(aA), lds_f32_off<4 * BF>(aB));
+                            const f32x2 v110 = pack2(lds_f32_off<4 * BF + 4>(aA), lds_f32_off<4 * BF + 4>(aB));
+                            const f32x2 v001 = pack2(lds_f32_off<4 * BF * BS>(aA), lds_f32_off<4 * BF * BS>(aB));
+                            const f32x2 v101 = pack2(lds_f32_off<4 * BF * BS + 4>(aA), lds_f32_off<4 * BF * BS + 4>(aB));
+                            const f32x2 v011 = pack2(lds_f32_off<4 * BF * BS + 4 * BF>(aA), lds_f32_off<4 * BF * BS + 4 * BF>(aB));
+                            const f32x2 v111 = pack2(lds_f32_off<4 * BF * BS + 4 * BF + 4>(aA), lds_f32_off<4 * BF * BS + 4 * BF + 4>(aB));
+                            const f32x2 a00 = fma2(wF, sub2(v100, v000), v000), a10 = fma2(wF, sub2(v110, v010), v010);
+                            const f32x2 a01 = fma2(wF, sub2(v101, v001), v001), a11 = fma2(wF, sub2(v111, v011), v011);
+                            const f32x2 b0 = fma2(wS, sub2(a10, a00), a00), b1 = fma2(wS, sub2(a11, a01), a01);
+                            float cA, cB;
+                            unpack2(fma2(wZ, sub2(b1, b0), b0), cA, cB);
+                            part += cA;
+                            part += cB;
+                        }
+                        if (j < n) {                                                                   // odd count: the last sample alone
+                            jf = (float)j;
+                            const f32x2 FS = fma2(pack2(jf, jf), pack2(sF, sS), pack2(F0, S0));
                             const float Z = fmaf(jf, sZ, Z0);
-                            const f32x2 rFS = add2(add2_rd(FS, magic2), neg_magic2);               // floors, exact
+                            const f32x2 rFS = add2(add2_rd(FS, magic2), neg_magic2);
                             const float rz = __fadd_rd(Z, FT_MAGIC) - FT_MAGIC;
                             const f32x2 wFS = sub2(FS, rFS);
                             const float wz = Z - rz;
                             float rf, rs, wf, ws;
                             unpack2(rFS, rf, rs); unpack2(wFS, wf, ws);
-                            const unsigned idx = (unsigned)__float2int_rn(fmaf(rz, pZf, fmaf(rs, pSf, rf)));
-                            const unsigned a0 = base_r + 4u * idx;
+                            const unsigned a0 = base_r + 4u * (unsigned)__float2int_rn(fmaf(rz, pZf, fmaf(rs, pSf, rf)));
                             // pairs over z: (lower plane, upper plane)
                             const f32x2 p00 = pack2(lds_f32_off<0>(a0), lds_f32_off<4 * BF * BS>(a0));
                             const f32x2 p10 = pack2(lds_f32_off<4>(a0), lds_f32_off<4 * BF * BS + 4>(a0));
                             const f32x2 p01 = pack2(lds_f32_off<4 * BF>(a0), lds_f32_off<4 * BF * BS + 4 * BF>(a0));
                             const f32x2 p11 = pack2(lds_f32_off<4 * BF + 4>(a0), lds_f32_off<4 * BF * BS + 4 * BF + 4>(a0));
                             const f32x2 wf2 = pack2(wf, wf), ws2 = pack2(ws, ws);
-                            const f32x2 a0x = fma2(wf2, sub2(p10, p00), p00), a1x = fma2(wf2, sub2(p11, p01), p01);   // (a00, a01), (a10, a11)
+                            const f32x2 a0x = fma2(wf2, sub2(p10, p00), p00), a1x = fma2(wf2, sub2(p11, p01), p01);
                             float b0, b1;
                             unpack2(fma2(ws2, sub2(a1x, a0x), a0x), b0, b1);
                             part += fmaf(wz, b1 - b0, b0);
                         }
                     } else {
 #pragma unroll 2
-                    for (int j = 0; j < n; ++j, jf += 1.f) {                        const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
+                    for (int j = 0; j < n; ++j, jf += 1.f) {
+                        const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
                         const float qf = __fadd_rd(F, FT_MAGIC), qs = __fadd_rd(S, FT_MAGIC), qz = __fadd_rd(Z, FT_MAGIC);
                         const float rf = qf - FT_MAGIC, rs = qs - FT_MAGIC, rz = qz - FT_MAGIC;      // floors, exact
                         const float wf = F - rf, ws = S - rs, wz = Z - rz;
