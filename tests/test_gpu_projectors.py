@@ -180,9 +180,11 @@ def test_host_buffer_entry_points_match_device_ones():
     assert np.array_equal(out_g.numpy(), g) and np.array_equal(out_f.numpy(), f)
 
 
-@pytest.mark.parametrize("cfg", [3, 4])
+@pytest.mark.parametrize("cfg", [3, 4, 5])
 def test_full_size_sampled_outputs(cfg):
-    """BASELINE sizes in the launch configuration bench.py times: oracle on sampled rays / voxels."""
+    """BASELINE sizes in the launch configuration bench.py times (cfg 4) and the 360-view stress configuration (cfg 5,
+    1024x768 detector: 2.4e11 samples per projector call, several int32 accumulation groups in P^T): oracle on sampled
+    rays / voxels."""
     w = syn.workload(cfg)
     G = w.geometry
     f0 = syn.voxelise(G, syn.ellipsoids_for(w))
