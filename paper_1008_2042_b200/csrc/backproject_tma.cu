@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(256) absmax_kernel(const float *__restrict__ g
 // LM 0 is the default (verified against the oracle by running this source under a CPU thread-per-CUDA-thread shim while
 // the GPU pool was closed; its 13.3 ms is the model's prediction from LM 1's measured 17.6 ms); CBCT_BT_LANES=1 selects LM 1.
 // The order in which a thread visits the samples of a chunk is free: integer sums do not depend on it.
-template <int BF, int BS, int LM>
+template <int BF, int BS, int LM, bool PK>
 __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                          const __grid_constant__ CUtensorMap map_y,
                                                                          const float *__restrict__ proj, int *__restrict__ acc_x,
@@ -152,6 +152,66 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
                 const unsigned base_r = smem_u32(buf0 + stage * box_elems);
                 const float pSf = (float)pS, pZf = (float)pZ;
                 const int n = jb - ja + 1;
+                if constexpr (PK) {
+                    // Packed pairs (FFMA2 / FADD2 / FMUL2), two consecutive samples per pair, as in forward_tma_kernel: the
+                    // positions, floors and fractions are bit-identical to the forward kernel's.  The thread starts `skew`
+                    // samples ahead (kept even, so pairs never straddle the wrap-around) and visits [s0, n) then [0, s0).
+                    const f32x2 sF2 = pack2(sF, sF), sS2 = pack2(sS, sS), sZ2 = pack2(sZ, sZ);
+                    const f32x2 F02 = pack2(F0, F0), S02 = pack2(S0, S0), Z02 = pack2(Z0, Z0);
+                    const f32x2 magic2 = pack2(FT_MAGIC, FT_MAGIC), neg_magic2 = pack2(-FT_MAGIC, -FT_MAGIC);
+                    const f32x2 pS2 = pack2(pSf, pSf), pZ2 = pack2(pZf, pZf), two2 = pack2(2.f, 2.f);
+                    const f32x2 gs2 = pack2(gs, gs), one2 = pack2(1.f, 1.f), round2 = pack2(BT_ROUND, BT_ROUND);
+                    const int s0 = (skew < n ? skew : skew % n) & ~1;
+#pragma unroll 1
+                    for (int seg = 0; seg < 2; ++seg) {
+                        int j = seg ? 0 : s0;
+                        const int end = seg ? s0 : n;
+                        f32x2 jj = pack2((float)j, (float)j + 1.f);
+#pragma unroll 1
+                        for (; j + 1 < end; j += 2, jj = add2(jj, two2)) {
+                            const f32x2 F = fma2(jj, sF2, F02), S = fma2(jj, sS2, S02), Z = fma2(jj, sZ2, Z02);
+                            const f32x2 rF = add2(add2_rd(F, magic2), neg_magic2), rS = add2(add2_rd(S, magic2), neg_magic2),
+                                        rZ = add2(add2_rd(Z, magic2), neg_magic2);
+                            const f32x2 wF = sub2(F, rF), wS = sub2(S, rS), wZ = sub2(Z, rZ);
+                            float ia, ib;
+                            unpack2(fma2(rZ, pZ2, fma2(rS, pS2, rF)), ia, ib);
+                            const unsigned aA = base_r + 4u * (unsigned)__float2int_rn(ia), aB = base_r + 4u * (unsigned)__float2int_rn(ib);
+                            // transposed lerp tree on both samples: split gs along z, then the slow axis, then the fast axis
+                            const f32x2 g1 = mul2(gs2, wZ), g0 = sub2(gs2, g1);
+                            const f32x2 g01 = mul2(g0, wS), g00 = sub2(g0, g01), g11 = mul2(g1, wS), g10 = sub2(g1, g11);
+                            const f32x2 oF = sub2(one2, wF);
+                            float cA, cB;
+#define CBCT_SCATTER2(OFF, G, W)                                                      \
+                            unpack2(fma2(G, W, round2), cA, cB);                      \
+                            red_s32_off<OFF>(aA, __float_as_int(cA) - BT_ROUND_BITS); \
+                            red_s32_off<OFF>(aB, __float_as_int(cB) - BT_ROUND_BITS);
+                            CBCT_SCATTER2(0, g00, oF) CBCT_SCATTER2(4, g00, wF)
+                            CBCT_SCATTER2(4 * BF, g01, oF) CBCT_SCATTER2(4 * BF + 4, g01, wF)
+                            CBCT_SCATTER2(4 * BF * BS, g10, oF) CBCT_SCATTER2(4 * BF * BS + 4, g10, wF)
+                            CBCT_SCATTER2(4 * BF * BS + 4 * BF, g11, oF) CBCT_SCATTER2(4 * BF * BS + 4 * BF + 4, g11, wF)
+#undef CBCT_SCATTER2
+                        }
+                        if (j < end) {                                     // odd count: the last sample of the segment alone
+                            const float jf = (float)j;
+                            const float F = fmaf(jf, sF, F0), S = fmaf(jf, sS, S0), Z = fmaf(jf, sZ, Z0);
+                            const float rf = __fadd_rd(F, FT_MAGIC) - FT_MAGIC, rs = __fadd_rd(S, FT_MAGIC) - FT_MAGIC,
+                                        rz = __fadd_rd(Z, FT_MAGIC) - FT_MAGIC;
+                            const float wf = F - rf, ws = S - rs, wz = Z - rz;
+                            const unsigned a0 = base_r + 4u * (unsigned)__float2int_rn(fmaf(rz, pZf, fmaf(rs, pSf, rf)));
+                            const float g1 = __fmul_rn(gs, wz), g0 = gs - g1;
+                            const float g01 = __fmul_rn(g0, ws), g00 = g0 - g01, g11 = __fmul_rn(g1, ws), g10 = g1 - g11;
+                            const float of = 1.f - wf;
+                            red_s32_off<0>(a0, round_mul(g00, of));
+                            red_s32_off<4>(a0, round_mul(g00, wf));
+                            red_s32_off<4 * BF>(a0, round_mul(g01, of));
+                            red_s32_off<4 * BF + 4>(a0, round_mul(g01, wf));
+                            red_s32_off<4 * BF * BS>(a0, round_mul(g10, of));
+                            red_s32_off<4 * BF * BS + 4>(a0, round_mul(g10, wf));
+                            red_s32_off<4 * BF * BS + 4 * BF>(a0, round_mul(g11, of));
+                            red_s32_off<4 * BF * BS + 4 * BF + 4>(a0, round_mul(g11, wf));
+                        }
+                    }
+                } else {
                 const float nf = (float)n;
                 float jf = (float)(skew < n ? skew : skew % n);        // start `skew` samples ahead, wrap around at n
 #pragma unroll 2
@@ -177,6 +237,7 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
                     red_s32_off<4 * BF * BS + 4 * BF + 4>(a0, round_mul(g11, wf));
                     jf += 1.f;
                     if (jf >= nf) jf -= nf;
+                }
                 }
             }
             fence_async_smem();                           // my shared-memory writes -> visible to the TMA unit
@@ -253,8 +314,14 @@ __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__
 
 typedef void (*ScatterKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, int *, const unsigned *, float, int,
                               float, int, int);
-static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm) {
-#define CBCT_SK(F, S, L) if (bf == F && bs == S && lm == L) return backproject_scatter_kernel<F, S, L>;
+// CBCT_BT_PACKED=0 selects the scalar instruction stream of the scatter kernel; default: packed pairs
+static bool scatter_packed() {
+    const char *e = getenv("CBCT_BT_PACKED");
+    return !(e && atoi(e) == 0);
+}
+static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm, bool pk) {
+#define CBCT_SK(F, S, L) \
+    if (bf == F && bs == S && lm == L) return pk ? backproject_scatter_kernel<F, S, L, true> : backproject_scatter_kernel<F, S, L, false>;
     CBCT_SK(24, 24, 0) CBCT_SK(40, 32, 0) CBCT_SK(40, 40, 0) CBCT_SK(56, 48, 0) CBCT_SK(56, 56, 0)      // plane pitch = 0 (mod 32)
     CBCT_SK(24, 22, 1) CBCT_SK(40, 30, 1) CBCT_SK(40, 38, 1) CBCT_SK(56, 46, 1) CBCT_SK(56, 54, 1)      // the forward kernel's boxes
 #undef CBCT_SK
@@ -329,12 +396,14 @@ void plan_backproject_tma(cbct_geometry *G) {
     }
     std::memcpy(G->bt_map_x, &mx, sizeof(mx));
     std::memcpy(G->bt_map_y, &my, sizeof(my));
-    ScatterKernel k = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm);
-    if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) !=
-                  cudaSuccess) {
-        (void)cudaGetLastError();
-        free_backproject_tma(G);
-        return;
+    for (int pk = 0; pk < 2; ++pk) {
+        ScatterKernel k = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, pk != 0);
+        if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) !=
+                      cudaSuccess) {
+            (void)cudaGetLastError();
+            free_backproject_tma(G);
+            return;
+        }
     }
     G->bt_ok = 1;
 }
@@ -345,7 +414,7 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
     CUtensorMap mx, my;
     std::memcpy(&mx, G->bt_map_x, sizeof(mx));
     std::memcpy(&my, G->bt_map_y, sizeof(my));
-    ScatterKernel kern = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm);
+    ScatterKernel kern = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, scatter_packed());
     if (!kern) return CBCT_E_UNSUPPORTED;
     CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_absmax, 0, sizeof(unsigned), st));
     absmax_kernel<<<592, 256, 0, st>>>(d_proj, (long long)G->n_rays, G->d_bt_absmax);

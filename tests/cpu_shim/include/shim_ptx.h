@@ -59,6 +59,7 @@ static inline f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
 }
 static inline f32x2 add2(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fadd_rn(a0, b0), __fadd_rn(a1, b1)); }
 static inline f32x2 sub2(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fadd_rn(a0, -b0), __fadd_rn(a1, -b1)); }
+static inline f32x2 mul2(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fmul_rn(a0, b0), __fmul_rn(a1, b1)); }
 static inline f32x2 add2_rd(f32x2 a, f32x2 b) { float a0, a1, b0, b1; unpack2(a, a0, a1); unpack2(b, b0, b1); return pack2(__fadd_rd(a0, b0), __fadd_rd(a1, b1)); }
 
 }  // namespace cbct

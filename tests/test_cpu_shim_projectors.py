@@ -101,18 +101,22 @@ def test_forward_fallback_kernels(monkeypatch):
         assert rel_l2_per_view(forward(G, f), op.forward(G, f.astype(np.float64))) <= TOL, (vox, pix)
 
 
+@pytest.mark.parametrize("packed", ["1", "0"])
 @pytest.mark.parametrize("lanes", ["0", "1"])
 @pytest.mark.parametrize("tma_mode", ["eager", "lazy"])
-def test_backproject_scatter_kernel(monkeypatch, lanes, tma_mode):
-    """both lane layouts of the TMA scatter kernel; signed input; lazy = tensor reductions read their shared-memory
-    box only at cp.async.bulk.wait_group (clearing the box too early loses the contributions)."""
+def test_backproject_scatter_kernel(monkeypatch, lanes, tma_mode, packed):
+    """both lane layouts and both instruction streams (packed pairs / scalar) of the TMA scatter kernel; signed input;
+    lazy = tensor reductions read their shared-memory box only at cp.async.bulk.wait_group (clearing the box too early
+    loses the contributions)."""
     monkeypatch.setenv("SHIM_TMA", tma_mode)
     monkeypatch.setenv("CBCT_BT_LANES", lanes)
+    monkeypatch.setenv("CBCT_BT_PACKED", packed)
     for G, seed in ((syn.workload(1).geometry, 34), (RAGGED_TMA, 72)):
         y = syn.uniform_projections(G, seed) - 0.4
         f = back(G, y)
-        assert any(k.startswith("cbct::backproject_scatter_kernel<") and k.endswith(f", {lanes}>") for k in sl.kernel_log())
-        assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, (lanes, tma_mode)
+        want = f", {lanes}, {'true' if packed == '1' else 'false'}>"
+        assert any(k.startswith("cbct::backproject_scatter_kernel<") and k.endswith(want) for k in sl.kernel_log())
+        assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, (lanes, tma_mode, packed)
 
 
 @pytest.mark.parametrize("impl", ["cell", "gather"])

@@ -226,6 +226,21 @@ def test_backproject_every_implementation_matches_oracle(monkeypatch, impl, lane
         assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, (impl, lanes, cfg)
 
 
+def test_backproject_scatter_packed_and_scalar_streams(monkeypatch):
+    """The scatter kernel's packed-pair instruction stream (FFMA2 / FADD2 / FMUL2, default) and the scalar one
+    (CBCT_BT_PACKED=0) visit the same samples with the same positions; both meet the bar, and they agree with each other
+    to the fixed-point unit (the weight products may round differently)."""
+    G = syn.workload(2).geometry
+    y = syn.uniform_projections(G, 36) - 0.4
+    ref = op.back_scatter(G, y.astype(np.float64))
+    out = {}
+    for pk in ("1", "0"):
+        monkeypatch.setenv("CBCT_BT_PACKED", pk)
+        out[pk], _ = gpu_back(G, y)
+        assert rel_l2(out[pk], ref) <= TOL, pk
+    assert rel_l2(out["1"], out["0"].astype(np.float64)) <= 1e-6
+
+
 def test_backproject_scatter_is_deterministic_and_scale_invariant():
     """The scatter kernel accumulates in fixed point relative to max|g|: the result is bit-identical from run
     to run (integer atomics are order-independent) and scales exactly with a power-of-two factor; a single
