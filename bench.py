@@ -150,6 +150,7 @@ def main():
     ap.add_argument("--workload", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernels-only", action="store_true", help="run P, P^T, fused TF 3x and exit (for ncu)")
+    ap.add_argument("--peaks", action="store_true", help="run the library's micro-benchmarks (cbct_microbench) and exit")
     ap.add_argument("--no-full-recon", action="store_true", help="skip the one-off 3-level 5/10/15 reconstruction timing")
     args = ap.parse_args()
 
@@ -178,6 +179,22 @@ def main():
     g = syn.analytic_projections(G, ells)
     if w.photons:
         g = syn.add_poisson_noise(g, w.photons, w.seed + rank)          # every replica its own noise draw
+
+    if args.peaks:
+        # per-SM rates that bound P / P^T; rates per clock are converted with the max SM clock for context
+        res = cb.microbench()
+        clk = load_peaks()["sm_max_mhz"] * 1e6
+        line = dict(peaks=True, n_sm=N_SM, sm_max_mhz=clk / 1e6)
+        for name, (rate, unit) in res.items():
+            line[name] = dict(value=rate, unit=unit)
+        line["derived"] = dict(
+            ffma_tinstr_s=res["ffma"][0] * 32 * N_SM * clk / 1e12, ffma2_tinstr_s=res["ffma2"][0] * 64 * N_SM * clk / 1e12,
+            lds_wavefronts_per_clk_sm=res["lds32"][0], atoms_wavefronts_per_clk_sm=res["atoms_add_s32"][0])
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, "gpurun_out", "peaks_local.json"), "w") as fh:
+            json.dump(line, fh, indent=1)
+        print(json.dumps(line), flush=True)
+        return
 
     if args.kernels_only:
         # short command for `ncu --set full`: 3 x (P, P^T, fused TF) on the workload, nothing else

@@ -121,6 +121,14 @@ int cbct_backproject_eq3(const cbct_geometry *geom, const float *d_proj, float *
 int cbct_siddon_forward(cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
 int cbct_siddon_backproject(cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
 
+/* Micro-benchmarks of the per-SM rates that bound the projector kernels on the device in use (the
+ * denominators MEASURED_PEAKS.json does not have).  Synchronises `stream`.  kind:
+ *   0 FFMA, 1 FFMA2 (packed pair), 2 LDS.32 conflict-free, 3 ATOMS.ADD.S32 conflict-free, 4 LDG.32 hitting L1
+ *     -> out[0] = warp instructions per clock per SM (clock64 inside the kernel, slowest warp of 32 per SM);
+ *   5 L2 read bandwidth on a 64 MB set -> out[0] = GB/s;   6 coalesced RED.ADD.S32 into a 64 MB set -> out[0] = 1e9 reductions/s.
+ * out[1] = seconds of the measured launch (CUDA events), out[2] = its work items. */
+int cbct_microbench(int kind, double out[3], void *stream);
+
 /* Host arithmetic only (no device needed): the fixed-point plan cbct_backproject uses for this geometry.
  *   max_weight_sum_per_view: upper bound on the sum of trilinear weights one voxel receives from one view;
  *   qb: contributions are rounded to multiples of max|g| / 2^qb;

@@ -23,7 +23,7 @@ EXPORTS = [
     "cbct_profile_begin", "cbct_profile_end",
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
-    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_forward", "cbct_siddon_backproject",
+    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_forward", "cbct_siddon_backproject", "cbct_microbench",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
@@ -84,6 +84,7 @@ def _declare(L):
     for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host", "cbct_backproject_eq3",
                  "cbct_siddon_forward", "cbct_siddon_backproject"):
         getattr(L, name).argtypes = [vp, fp, fp, vp]
+    L.cbct_microbench.argtypes = [ip, C.POINTER(C.c_double), vp]
     L.cbct_backproject_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                                     C.POINTER(C.c_double)]
     L.cbct_cgls_create.argtypes = [vp, C.POINTER(vp)]
@@ -172,6 +173,21 @@ def make_desc(geom):
                      geom.nu, geom.nv, geom.du, geom.dv, geom.u0, geom.v0, geom.sad, geom.sdd,
                      len(ang), ang.ctypes.data_as(C.POINTER(C.c_double)), float(getattr(geom, "step_mm", 0.0)))
     return d, ang
+
+
+MICROBENCH_KINDS = {0: ("ffma", "warp-instr/clk/SM"), 1: ("ffma2", "warp-instr/clk/SM"), 2: ("lds32", "warp-instr/clk/SM"),
+                    3: ("atoms_add_s32", "warp-instr/clk/SM"), 4: ("ldg32_l1_hit", "warp-instr/clk/SM"),
+                    5: ("l2_read_64MB", "GB/s"), 6: ("l2_red_add_s32", "Gred/s")}
+
+
+def microbench(stream=None):
+    """{name: (rate, unit)} of cbct_microbench for every kind."""
+    res = {}
+    for kind, (name, unit) in MICROBENCH_KINDS.items():
+        out = (C.c_double * 3)()
+        _check(lib().cbct_microbench(kind, out, _stream(stream)), "cbct_microbench")
+        res[name] = (out[0], unit)
+    return res
 
 
 def backproject_fixed_point_plan(geom):

@@ -69,6 +69,13 @@ __device__ __forceinline__ void red_s32_off(unsigned addr, int v) {
     asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(v) : "memory");
 }
 
+// ---- global load that bypasses L1 (micro-benchmark of the L2) ----------------------------------------------------------------
+__device__ __forceinline__ float4 ldg_cg_f4(const float4 *p) {
+    float4 v;
+    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
 // ---- packed fp32 pairs (sm_100: FFMA2 / FADD2 work on two fp32 lanes of a 64-bit register pair per instruction) -----------
 // Each lane is an IEEE fp32 operation with the stated rounding: results are bit-identical to the scalar instructions.
 typedef unsigned long long f32x2;

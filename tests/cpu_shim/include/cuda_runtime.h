@@ -110,6 +110,7 @@ uint64_t warp_collective(unsigned mask, WarpOp op, uint64_t payload, int arg);
 #define SHIM_LAUNCH(...) ::shim::launch_kernel(__VA_ARGS__)
 static inline void __syncthreads() { shim::syncthreads(); }
 static inline void __syncwarp(unsigned mask = 0xffffffffu) { shim::warp_collective(mask, shim::W_BALLOT, 0, 0); }
+static inline long long clock64() { return (long long)__builtin_ia32_rdtsc(); }
 static inline void __threadfence() { __atomic_thread_fence(__ATOMIC_SEQ_CST); }
 
 static inline int __reduce_min_sync(unsigned m, int v) { return (int)shim::warp_collective(m, shim::W_MIN_S32, (uint64_t)(int64_t)v, 0); }

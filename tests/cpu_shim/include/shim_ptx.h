@@ -48,6 +48,8 @@ static inline void red_s32(unsigned addr, int v) { shim::bank_record(addr, 1); *
 template <int OFF>
 static inline void red_s32_off(unsigned addr, int v) { red_s32(addr + (unsigned)OFF, v); }
 
+static inline float4 ldg_cg_f4(const float4 *p) { shim::check_align(p, 16, "ld.global.cg.v4"); return *p; }
+
 // packed fp32 pairs: two independent IEEE operations
 typedef unsigned long long f32x2;
 static inline f32x2 pack2(float lo, float hi) { f32x2 r; float v[2] = {lo, hi}; std::memcpy(&r, v, 8); return r; }
