@@ -5,6 +5,9 @@
 // wavefronts, L1-hit LDG, L2 read bandwidth on a 64 MB set, and L2 integer reductions (RED.ADD.S32).
 // Rates per SM are measured with clock64() inside the kernel (one CTA of 1024 threads per SM, the slowest warp counts),
 // so they do not depend on knowing the SM clock; bandwidths are measured with CUDA events on the launching stream.
+#include <algorithm>
+#include <cstdlib>
+
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -105,15 +108,27 @@ extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
     if (!out || kind < 0 || kind > 6) return CBCT_E_INVALID;
     CBCT_TRY(device_supported());
     cudaStream_t st = as_stream(stream);
-    const int n_sm = 148, iters = 2000;
-    long long *d_cycles = nullptr;
-    float *d_sink = nullptr, *d_buf = nullptr;
+    // CBCT_MB_ITERS shortens the timed loops (host-side checks of the kernels; the default is what is reported)
+    const int n_sm = 148, iters = getenv("CBCT_MB_ITERS") ? std::max(1, atoi(getenv("CBCT_MB_ITERS"))) : 2000;
+    const int reps_rd = iters >= 2000 ? 20 : 1, reps_red = iters >= 2000 ? 4 : 1;
+    struct Scratch {                                                   // released on every return path
+        long long *cycles = nullptr;
+        float *sink = nullptr, *buf = nullptr;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        ~Scratch() {
+            if (e0) cudaEventDestroy(e0);
+            if (e1) cudaEventDestroy(e1);
+            cudaFree(cycles); cudaFree(sink); cudaFree(buf);
+        }
+    } sc;
+    long long *&d_cycles = sc.cycles;
+    float *&d_sink = sc.sink, *&d_buf = sc.buf;
     const size_t set_bytes = (size_t)64 << 20;
     CBCT_CUDA_TRY(cudaMalloc(&d_cycles, sizeof(long long) * n_sm * 32));
     CBCT_CUDA_TRY(cudaMalloc(&d_sink, 256));
     CBCT_CUDA_TRY(cudaMalloc(&d_buf, set_bytes));
     CBCT_CUDA_TRY(cudaMemsetAsync(d_buf, 0, set_bytes, st));
-    cudaEvent_t e0, e1;
+    cudaEvent_t &e0 = sc.e0, &e1 = sc.e1;
     CBCT_CUDA_TRY(cudaEventCreate(&e0));
     CBCT_CUDA_TRY(cudaEventCreate(&e1));
     double work = 0;
@@ -125,8 +140,8 @@ extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
             case 2: mb_smem_kernel<2><<<n_sm, 1024, 0, st>>>(iters, d_cycles, d_sink); break;
             case 3: mb_smem_kernel<3><<<n_sm, 1024, 0, st>>>(iters, d_cycles, d_sink); break;
             case 4: mb_ldg_kernel<<<n_sm, 1024, 0, st>>>(iters, d_buf, d_cycles, d_sink); break;
-            case 5: mb_l2_read_kernel<<<n_sm * 8, 256, 0, st>>>(reinterpret_cast<const float4 *>(d_buf), (long long)(set_bytes / 16), 20, d_sink); break;
-            case 6: mb_l2_red_kernel<<<n_sm * 8, 256, 0, st>>>(reinterpret_cast<int *>(d_buf), (long long)(set_bytes / 4), 4); break;
+            case 5: mb_l2_read_kernel<<<n_sm * 8, 256, 0, st>>>(reinterpret_cast<const float4 *>(d_buf), (long long)(set_bytes / 16), reps_rd, d_sink); break;
+            case 6: mb_l2_red_kernel<<<n_sm * 8, 256, 0, st>>>(reinterpret_cast<int *>(d_buf), (long long)(set_bytes / 4), reps_red); break;
         }
         CBCT_LAUNCH_CHECK();
         CBCT_CUDA_TRY(cudaEventRecord(e1, st));
@@ -142,15 +157,13 @@ extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
         work = 32.0 * iters * MB_UNROLL;                                // warp instructions per SM
         out[0] = work / (double)worst;                                  // warp instructions per clock per SM
     } else if (kind == 5) {
-        work = 20.0 * (double)set_bytes;
+        work = (double)reps_rd * (double)set_bytes;
         out[0] = work / (ms * 1e-3) / 1e9;                              // GB/s
     } else {
-        work = 4.0 * (double)(set_bytes / 4);
+        work = (double)reps_red * (double)(set_bytes / 4);
         out[0] = work / (ms * 1e-3) / 1e9;                              // G reductions per second
     }
     out[1] = ms * 1e-3;
     out[2] = work;
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(d_cycles); cudaFree(d_sink); cudaFree(d_buf);
     return CBCT_OK;
 }

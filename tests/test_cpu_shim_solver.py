@@ -126,3 +126,15 @@ def test_multigrid_a2_driver_two_levels():
     ref = osv.multigrid_a2(make_ops, G.vol_shape, g.astype(np.float64), 2, n_outer, n_cgls, mu)
     out = sl.tf_reconstruct_volume(G, sl.dev(g), 2, n_outer, n_cgls, mu, True).numpy()
     assert rel(out, ref) <= 1e-4
+
+
+def test_microbench_kernels_stay_in_bounds(monkeypatch):
+    """cbct_microbench (SURVEY.md §8(d) denominators) with its timed loops shortened: every kernel runs under the shim's
+    guards and alignment checks; the rates themselves mean nothing on the host."""
+    import ctypes as C
+    monkeypatch.setenv("CBCT_MB_ITERS", "1")
+    for kind in range(7):
+        out = (C.c_double * 3)()
+        sl.check(sl.lib().cbct_microbench(kind, out, None), f"cbct_microbench({kind})")
+        assert out[2] > 0
+    assert sl.lib().cbct_microbench(7, out, None) == -1
