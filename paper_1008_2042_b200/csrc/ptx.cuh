@@ -69,6 +69,18 @@ __device__ __forceinline__ void red_s32_off(unsigned addr, int v) {
     asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(v) : "memory");
 }
 
+// the eight corner reductions of one trilinear sample (box pitches BF, BF * BS) for the lanes whose predicate holds; the
+// others sit all eight instructions out under one branch
+template <int BF, int BS>
+__device__ __forceinline__ void red_s32_x8_if(unsigned addr, const int (&v)[8], bool pred) {
+    if (pred) {
+        red_s32_off<0>(addr, v[0]);                    red_s32_off<4>(addr, v[1]);
+        red_s32_off<4 * BF>(addr, v[2]);               red_s32_off<4 * BF + 4>(addr, v[3]);
+        red_s32_off<4 * BF * BS>(addr, v[4]);          red_s32_off<4 * BF * BS + 4>(addr, v[5]);
+        red_s32_off<4 * BF * BS + 4 * BF>(addr, v[6]); red_s32_off<4 * BF * BS + 4 * BF + 4>(addr, v[7]);
+    }
+}
+
 // ---- global load that bypasses L1 (micro-benchmark of the L2) ----------------------------------------------------------------
 __device__ __forceinline__ float4 ldg_cg_f4(const float4 *p) {
     float4 v;

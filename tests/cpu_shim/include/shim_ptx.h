@@ -48,6 +48,14 @@ static inline void red_s32(unsigned addr, int v) { shim::bank_record(addr, 1); *
 template <int OFF>
 static inline void red_s32_off(unsigned addr, int v) { red_s32(addr + (unsigned)OFF, v); }
 
+template <int BF, int BS>
+static inline void red_s32_x8_if(unsigned addr, const int (&v)[8], bool pred) {
+    const unsigned off[8] = {0, 4, 4 * BF, 4 * BF + 4, 4 * BF * BS, 4 * BF * BS + 4, 4 * BF * BS + 4 * BF, 4 * BF * BS + 4 * BF + 4};
+    for (int i = 0; i < 8; ++i) {
+        if (pred) red_s32(addr + off[i], v[i]);
+        else shim::bank_record(0xffffffffu, 2);          // keeps the lane's instruction ordinal aligned with its warp
+    }
+}
 static inline float4 ldg_cg_f4(const float4 *p) { shim::check_align(p, 16, "ld.global.cg.v4"); return *p; }
 
 // packed fp32 pairs: two independent IEEE operations

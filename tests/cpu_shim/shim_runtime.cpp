@@ -256,6 +256,7 @@ void bank_record(unsigned addr, unsigned kind) {
     if (!g_bank_on) return;
     Worker *w = tw;
     Fiber &f = w->fibers[w->cur];
+    if (kind == 2) { ++f.seq; return; }                 // a lane predicated off: the ordinal advances, no request
     w->bank.push_back(BankRec{(unsigned)f.lin >> 5, (w->epoch << 18) | (f.seq++ & 0x3ffff), addr, kind});
 }
 static void bank_flush(Worker *w) {
