@@ -89,15 +89,15 @@ __device__ __forceinline__ SiddonRay siddon_setup(const DevGeom &g, int view, in
 
 // The traversal.  `visit(linear_index, length)` is called once per voxel crossing of positive or zero length.
 template <class Visit>
-__device__ __forceinline__ void siddon_walk(const SiddonRay &s, long long sx, long long sy, long long sz, Visit visit) {
+__device__ __forceinline__ void siddon_walk(const SiddonRay &s, int sx, int sy, int sz, Visit visit) {
     int ix = s.i[0], iy = s.i[1], iz = s.i[2];
     // next plane on each axis: the upper face of the current voxel when moving up, the lower face when moving down
     // (numbered relative to p0, see siddon_setup)
     float px = (float)(ix + (s.dir[0] > 0) - s.p0[0]), py = (float)(iy + (s.dir[1] > 0) - s.p0[1]), pz = (float)(iz + (s.dir[2] > 0) - s.p0[2]);
     const float dxf = (float)s.dir[0], dyf = (float)s.dir[1], dzf = (float)s.dir[2];
     float tx = fmaf(px, s.ib[0], s.k[0]), ty = fmaf(py, s.ib[1], s.k[1]), tz = fmaf(pz, s.ib[2], s.k[2]);
-    long long lin = ix * sx + iy * sy + iz * sz;
-    const long long dsx = s.dir[0] * sx, dsy = s.dir[1] * sy, dsz = s.dir[2] * sz;
+    int lin = ix * sx + iy * sy + iz * sz;                                                   // n_vox < 2^31 (checked at the entry points)
+    const int dsx = s.dir[0] * sx, dsy = s.dir[1] * sy, dsz = s.dir[2] * sz;
     float tau = s.tau;
     const int max_steps = s.n[0] + s.n[1] + s.n[2] + 3;                                      // a ray crosses at most that many planes
     for (int step = 0; step < max_steps; ++step) {
@@ -129,8 +129,8 @@ __global__ void __launch_bounds__(256) siddon_forward_kernel(DevGeom g, const fl
         const double2 cs = g.view_cs[view];
         const bool yfast = fabs(cs.x) > fabs(cs.y);                                          // rays run along x: read vol[z][x][y]
         const float *src = yfast ? volT : vol;
-        const long long sx = yfast ? g.ny : 1, sy = yfast ? 1 : g.nx, sz = (long long)g.nx * g.ny;
-        siddon_walk(s, sx, sy, sz, [&](long long lin, float len) { acc = fmaf(len, __ldg(src + lin), acc); });
+        const int sx = yfast ? g.ny : 1, sy = yfast ? 1 : g.nx, sz = g.nx * g.ny;
+        siddon_walk(s, sx, sy, sz, [&](int lin, float len) { acc = fmaf(len, __ldg(src + lin), acc); });
     }
     proj[((size_t)view * g.nv + iv) * g.nu + iu] = acc;
 }
@@ -149,8 +149,8 @@ __global__ void __launch_bounds__(256) siddon_scatter_kernel(DevGeom g, const fl
     const double2 cs = g.view_cs[view];
     const bool yfast = fabs(cs.x) > fabs(cs.y);
     int *dst = yfast ? acc_y : acc_x;
-    const long long sx = yfast ? g.ny : 1, sy = yfast ? 1 : g.nx, sz = (long long)g.nx * g.ny;
-    siddon_walk(s, sx, sy, sz, [&](long long lin, float len) {
+    const int sx = yfast ? g.ny : 1, sy = yfast ? 1 : g.nx, sz = g.nx * g.ny;
+    siddon_walk(s, sx, sy, sz, [&](int lin, float len) {
         const int q = __float2int_rn(gs * len);
         if (q) atomicAdd(dst + lin, q);                                                      // result unused: RED.ADD.S32
     });
@@ -199,6 +199,7 @@ using namespace cbct;
 
 extern "C" int cbct_siddon_forward(cbct_geometry *G, const float *d_vol, float *d_proj, void *stream) {
     if (!G || !d_vol || !d_proj) return CBCT_E_INVALID;
+    if (G->n_vox > 0x7fffffffLL) return CBCT_E_UNSUPPORTED;           // 32-bit voxel indices in the traversal
     CBCT_TRY(device_supported());
     CBCT_TRY(siddon_workspace(G, false));
     const DevGeom &g = G->dg;
@@ -216,6 +217,7 @@ extern "C" int cbct_siddon_forward(cbct_geometry *G, const float *d_vol, float *
 
 extern "C" int cbct_siddon_backproject(cbct_geometry *G, const float *d_proj, float *d_vol, void *stream) {
     if (!G || !d_vol || !d_proj) return CBCT_E_INVALID;
+    if (G->n_vox > 0x7fffffffLL) return CBCT_E_UNSUPPORTED;
     CBCT_TRY(device_supported());
     CBCT_TRY(siddon_workspace(G, true));
     const DevGeom &g = G->dg;
