@@ -2,6 +2,8 @@
 """bench.py -- whole-hot-path benchmark of the B200 CBCT library (one JSON line on stdout).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 4]
+    python bench.py --kernels-only      # P, P^T, fused TF, Siddon pair a few times (the command ncu wraps)
+    python bench.py --peaks             # cbct_microbench: the per-SM rates that bound P / P^T on this device
 
 A *step* is one pass of the whole hot path (every row) over one batch of synthetic
 input at BASELINE.json's paper-size config (512x512x70 volume, 40 views of 512x384, step 0.25 mm):
