@@ -125,6 +125,7 @@ int cbct_siddon_backproject(cbct_geometry *geom, const float *d_proj, float *d_v
  * denominators MEASURED_PEAKS.json does not have).  Synchronises `stream`.  kind:
  *   0 FFMA, 1 FFMA2 (packed pair), 2 LDS.32 conflict-free, 3 ATOMS.ADD.S32 conflict-free, 4 LDG.32 hitting L1
  *     -> out[0] = warp instructions per clock per SM (clock64 inside the kernel, slowest warp of 32 per SM);
+ *   7 ATOMS.ADD.64 conflict-free (256 contiguous bytes per instruction) -> warp instructions per clock per SM;
  *   5 L2 read bandwidth on a 64 MB set -> out[0] = GB/s;   6 coalesced RED.ADD.S32 into a 64 MB set -> out[0] = 1e9 reductions/s.
  * out[1] = seconds of the measured launch (CUDA events), out[2] = its work items. */
 int cbct_microbench(int kind, double out[3], void *stream);

@@ -177,7 +177,7 @@ def make_desc(geom):
 
 MICROBENCH_KINDS = {0: ("ffma", "warp-instr/clk/SM"), 1: ("ffma2", "warp-instr/clk/SM"), 2: ("lds32", "warp-instr/clk/SM"),
                     3: ("atoms_add_s32", "warp-instr/clk/SM"), 4: ("ldg32_l1_hit", "warp-instr/clk/SM"),
-                    5: ("l2_read_64MB", "GB/s"), 6: ("l2_red_add_s32", "Gred/s")}
+                    5: ("l2_read_64MB", "GB/s"), 6: ("l2_red_add_s32", "Gred/s"), 7: ("atoms_add_u64", "warp-instr/clk/SM")}
 
 
 def microbench(stream=None):

@@ -45,12 +45,13 @@ __global__ void __launch_bounds__(1024) mb_fma_kernel(int iters, float seed, lon
 }
 
 // kind 2: LDS.32, kind 3: ATOMS.ADD.S32; lane l touches word (l + k) of a 4 KB window: 32 distinct banks per instruction
+// kind 7: ATOMS.ADD.64, lane l touches the 8-byte word l of an 8 KB window (256 contiguous bytes per instruction)
 template <int KIND>
 __global__ void __launch_bounds__(1024) mb_smem_kernel(int iters, long long *cycles, float *sink) {
-    __shared__ int buf[1024 + 64];
-    for (int i = threadIdx.x; i < 1024 + 64; i += blockDim.x) buf[i] = i;
+    __shared__ __align__(16) int buf[2048 + 128];
+    for (int i = threadIdx.x; i < 2048 + 128; i += blockDim.x) buf[i] = i;
     __syncthreads();
-    const unsigned base = smem_u32(buf) + 4u * (threadIdx.x & 31);
+    const unsigned base = smem_u32(buf) + (KIND == 7 ? 8u : 4u) * (threadIdx.x & 31);
     float acc = 0.f;
     const long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
@@ -58,7 +59,8 @@ __global__ void __launch_bounds__(1024) mb_smem_kernel(int iters, long long *cyc
 #pragma unroll
         for (int u = 0; u < MB_UNROLL; ++u) {
             if (KIND == 2) acc += lds_f32(a + 128u * (u & 15));
-            else red_s32(a + 128u * (u & 15), 1);
+            else if (KIND == 3) red_s32(a + 128u * (u & 15), 1);
+            else red_u64(a + 256u * (u & 15), 1ull);
         }
     }
     const long long t1 = clock64();
@@ -105,7 +107,7 @@ using namespace cbct;
 
 // out[0] = the rate, out[1] = seconds (event time of the measured launch), out[2] = work items of that launch
 extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
-    if (!out || kind < 0 || kind > 6) return CBCT_E_INVALID;
+    if (!out || kind < 0 || kind > 7) return CBCT_E_INVALID;
     CBCT_TRY(device_supported());
     cudaStream_t st = as_stream(stream);
     // CBCT_MB_ITERS shortens the timed loops (host-side checks of the kernels; the default is what is reported)
@@ -139,6 +141,7 @@ extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
             case 1: mb_fma_kernel<1><<<n_sm, 1024, 0, st>>>(iters, 1.5f, d_cycles, d_sink); break;
             case 2: mb_smem_kernel<2><<<n_sm, 1024, 0, st>>>(iters, d_cycles, d_sink); break;
             case 3: mb_smem_kernel<3><<<n_sm, 1024, 0, st>>>(iters, d_cycles, d_sink); break;
+            case 7: mb_smem_kernel<7><<<n_sm, 1024, 0, st>>>(iters, d_cycles, d_sink); break;
             case 4: mb_ldg_kernel<<<n_sm, 1024, 0, st>>>(iters, d_buf, d_cycles, d_sink); break;
             case 5: mb_l2_read_kernel<<<n_sm * 8, 256, 0, st>>>(reinterpret_cast<const float4 *>(d_buf), (long long)(set_bytes / 16), reps_rd, d_sink); break;
             case 6: mb_l2_red_kernel<<<n_sm * 8, 256, 0, st>>>(reinterpret_cast<int *>(d_buf), (long long)(set_bytes / 4), reps_red); break;
@@ -149,7 +152,7 @@ extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
     CBCT_CUDA_TRY(cudaEventSynchronize(e1));
     float ms = 0.f;
     CBCT_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
-    if (kind <= 4) {
+    if (kind <= 4 || kind == 7) {
         std::vector<long long> cyc(n_sm * 32);
         CBCT_CUDA_TRY(cudaMemcpy(cyc.data(), d_cycles, sizeof(long long) * cyc.size(), cudaMemcpyDeviceToHost));
         long long worst = 1;

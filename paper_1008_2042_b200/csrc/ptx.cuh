@@ -69,6 +69,9 @@ __device__ __forceinline__ void red_s32_off(unsigned addr, int v) {
     asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(v) : "memory");
 }
 
+__device__ __forceinline__ void red_u64(unsigned addr, unsigned long long v) {
+    asm volatile("red.shared.add.u64 [%0], %1;" ::"r"(addr), "l"(v) : "memory");
+}
 // the eight corner reductions of one trilinear sample (box pitches BF, BF * BS) for the lanes whose predicate holds; the
 // others sit all eight instructions out under one branch
 template <int BF, int BS>

@@ -48,6 +48,7 @@ static inline void red_s32(unsigned addr, int v) { shim::bank_record(addr, 1); *
 template <int OFF>
 static inline void red_s32_off(unsigned addr, int v) { red_s32(addr + (unsigned)OFF, v); }
 
+static inline void red_u64(unsigned addr, unsigned long long v) { *static_cast<unsigned long long *>(shim::shared_ptr_of(addr, 8, "red.shared.add.u64")) += v; }
 template <int BF, int BS>
 static inline void red_s32_x8_if(unsigned addr, const int (&v)[8], bool pred) {
     const unsigned off[8] = {0, 4, 4 * BF, 4 * BF + 4, 4 * BF * BS, 4 * BF * BS + 4, 4 * BF * BS + 4 * BF, 4 * BF * BS + 4 * BF + 4};

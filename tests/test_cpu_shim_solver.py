@@ -133,8 +133,8 @@ def test_microbench_kernels_stay_in_bounds(monkeypatch):
     guards and alignment checks; the rates themselves mean nothing on the host."""
     import ctypes as C
     monkeypatch.setenv("CBCT_MB_ITERS", "1")
-    for kind in range(7):
+    for kind in range(8):
         out = (C.c_double * 3)()
         sl.check(sl.lib().cbct_microbench(kind, out, None), f"cbct_microbench({kind})")
         assert out[2] > 0
-    assert sl.lib().cbct_microbench(7, out, None) == -1
+    assert sl.lib().cbct_microbench(8, out, None) == -1
