@@ -121,6 +121,11 @@ int cbct_backproject_eq3(const cbct_geometry *geom, const float *d_proj, float *
 int cbct_siddon_forward(cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
 int cbct_siddon_backproject(cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
 
+/* Host arithmetic only: the fixed-point plan of cbct_siddon_backproject.  max_path_sum_per_view bounds the path length
+ * (mm) one voxel can collect from one view: (pixels its shadow can touch at the nearest depth) x (voxel diagonal);
+ * views_per_group * max_path_sum_per_view * 2^qb < 2^31.  CBCT_E_UNSUPPORTED if no qb >= 9 fits one view. */
+int cbct_siddon_fixed_point_plan(const cbct_geometry_desc *desc, int32_t *qb, int32_t *views_per_group, double *max_path_sum_per_view);
+
 /* Micro-benchmarks of the per-SM rates that bound the projector kernels on the device in use (the
  * denominators MEASURED_PEAKS.json does not have).  Synchronises `stream`.  kind:
  *   0 FFMA, 1 FFMA2 (packed pair), 2 LDS.32 conflict-free, 3 ATOMS.ADD.S32 conflict-free, 4 LDG.32 hitting L1

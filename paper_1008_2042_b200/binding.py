@@ -23,7 +23,7 @@ EXPORTS = [
     "cbct_profile_begin", "cbct_profile_end",
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
-    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_forward", "cbct_siddon_backproject", "cbct_microbench",
+    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_forward", "cbct_siddon_backproject", "cbct_siddon_fixed_point_plan", "cbct_microbench",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
@@ -84,6 +84,8 @@ def _declare(L):
     for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host", "cbct_backproject_eq3",
                  "cbct_siddon_forward", "cbct_siddon_backproject"):
         getattr(L, name).argtypes = [vp, fp, fp, vp]
+    L.cbct_siddon_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                               C.POINTER(C.c_double)]
     L.cbct_microbench.argtypes = [ip, C.POINTER(C.c_double), vp]
     L.cbct_backproject_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                                     C.POINTER(C.c_double)]
@@ -196,6 +198,14 @@ def backproject_fixed_point_plan(geom):
     qb, grp, w = C.c_int32(), C.c_int32(), C.c_double()
     _check(lib().cbct_backproject_fixed_point_plan(C.byref(d), C.byref(qb), C.byref(grp), C.byref(w)),
            "cbct_backproject_fixed_point_plan")
+    return qb.value, grp.value, w.value
+
+
+def siddon_fixed_point_plan(geom):
+    """(qb, views_per_group, max_path_sum_per_view) of cbct_siddon_backproject for this geometry; host only."""
+    d, keep = make_desc(geom)
+    qb, grp, w = C.c_int32(), C.c_int32(), C.c_double()
+    _check(lib().cbct_siddon_fixed_point_plan(C.byref(d), C.byref(qb), C.byref(grp), C.byref(w)), "cbct_siddon_fixed_point_plan")
     return qb.value, grp.value, w.value
 
 

@@ -157,6 +157,7 @@ void free_backproject_tma(cbct_geometry *g);
 bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int *qb, int *views_per_group, double *w_view);
 int launch_backproject_tma(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
 void free_siddon(cbct_geometry *g);
+bool siddon_fixed_point_plan(const cbct_geometry_desc &d, double R, int *qb, int *views_per_group, double *w_view);
 // kernels launched from more than one translation unit
 __global__ void transpose_vol_kernel(const float *__restrict__ v, float *__restrict__ vT, int nx, int ny);      // forward_tma.cu
 __global__ void absmax_kernel(const float *__restrict__ g, long long n, unsigned *out);                        // backproject_tma.cu

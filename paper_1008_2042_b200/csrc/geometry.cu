@@ -230,6 +230,19 @@ extern "C" int cbct_backproject_fixed_point_plan(const cbct_geometry_desc *desc,
     return CBCT_OK;
 }
 
+extern "C" int cbct_siddon_fixed_point_plan(const cbct_geometry_desc *desc, int32_t *qb, int32_t *views_per_group,
+                                           double *max_path_sum_per_view) {
+    double R = 0, step = 0;
+    CBCT_TRY(validate(desc, &R, &step));
+    int q = 0, grp = 0;
+    double w = 0;
+    if (!siddon_fixed_point_plan(*desc, R, &q, &grp, &w)) return CBCT_E_UNSUPPORTED;
+    if (qb) *qb = q;
+    if (views_per_group) *views_per_group = grp;
+    if (max_path_sum_per_view) *max_path_sum_per_view = w;
+    return CBCT_OK;
+}
+
 extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     if (!G) return CBCT_OK;
     cudaFree(G->d_view_cs);

@@ -165,22 +165,32 @@ static double siddon_weight_bound(const cbct_geometry_desc &d, double R) {
     return nu_ * nv_ * std::sqrt(d.dx * d.dx + d.dy * d.dy + d.dz * d.dz);
 }
 
+// 2^qb units per max|g| mm; views_per_group * w * 2^qb < 2^31.  Prefer all views in one group at qb >= 18, else groups of
+// views at qb = 18 (the finalize pass accumulates in fp32 between groups), else the largest qb that fits one view.
+// Host arithmetic only (exported as cbct_siddon_fixed_point_plan).
+bool siddon_fixed_point_plan(const cbct_geometry_desc &d, double R, int *qb_out, int *group_out, double *w_out) {
+    const double w = siddon_weight_bound(d, R);
+    const auto cap = [&](int bits) { return std::ldexp(1.0, 31 - bits) / w; };
+    int qb = 22;
+    while (qb > 18 && cap(qb) < (double)d.n_views) --qb;
+    while (qb > 8 && cap(qb) < 1.0) --qb;
+    if (cap(qb) < 1.0) return false;
+    *qb_out = qb;
+    *group_out = (int)std::fmin((double)d.n_views, std::floor(cap(qb)));
+    *w_out = w;
+    return true;
+}
+
 static int siddon_workspace(cbct_geometry *G, bool need_acc) {
     if (!G->d_sd_volT) {
         CBCT_CUDA_TRY(cudaMalloc(&G->d_sd_volT, sizeof(float) * G->n_vox));
         G->workspace_bytes += sizeof(float) * G->n_vox;
     }
     if (need_acc && !G->d_sd_acc) {
-        const double w = siddon_weight_bound(G->desc, G->R);
-        // 2^qb units per max|g| mm; views_per_group * w * 2^qb < 2^31.  Prefer all views in one group at qb >= 18, else
-        // groups of views at qb = 18 (finalize accumulates in fp32 between groups), else the largest qb that fits one view.
-        const auto cap = [&](int bits) { return std::ldexp(1.0, 31 - bits) / w; };
-        int qb = 22;
-        while (qb > 18 && cap(qb) < (double)G->desc.n_views) --qb;
-        while (qb > 8 && cap(qb) < 1.0) --qb;
-        if (cap(qb) < 1.0) return CBCT_E_UNSUPPORTED;
-        G->sd_qb = qb;
-        G->sd_group = (int)std::fmin((double)G->desc.n_views, std::floor(cap(qb)));
+        int qb = 0, group = 0;
+        double w = 0;
+        if (!siddon_fixed_point_plan(G->desc, G->R, &qb, &group, &w)) return CBCT_E_UNSUPPORTED;
+        G->sd_qb = qb; G->sd_group = group;
         CBCT_CUDA_TRY(cudaMalloc(&G->d_sd_acc, sizeof(int) * 2 * G->n_vox));
         CBCT_CUDA_TRY(cudaMalloc(&G->d_sd_absmax, sizeof(unsigned)));
         G->workspace_bytes += sizeof(int) * 2 * G->n_vox + sizeof(unsigned);

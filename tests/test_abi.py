@@ -90,6 +90,26 @@ def test_backproject_fixed_point_plan_bounds_the_oracle_weight_sums():
     assert binding.lib().cbct_backproject_fixed_point_plan(ctypes.byref(d), None, None, None) == binding.CBCT_E_INVALID
 
 
+def test_siddon_fixed_point_plan_bounds_the_oracle_path_sums():
+    """cbct_siddon_backproject accumulates g * length in int32: the planned bound on the path length one voxel collects
+    from one view must hold against the oracle (P_siddon^T of a one-view all-ones projection IS that sum)."""
+    from dataclasses import replace
+    from oracle import projector as op
+    G1 = syn.workload(1).geometry
+    cases = [G1, replace(G1, nu=24, nv=8, du=12.8, dv=12.8), replace(G1, ox=30.0, oy=-20.0, oz=10.0), replace(G1, nu=384, du=0.8),
+             syn.Geometry(24, 20, 40, 4.0, 4.0, 0.5, 28, 64, 5.0, 8.0, 1000.0, 1500.0, (0.2, 1.3, 2.9, 4.1, 5.6), oz=3.0)]
+    for G in cases:
+        qb, group, w_view = binding.siddon_fixed_point_plan(G)
+        assert 9 <= qb <= 22 and 1 <= group <= G.n_views
+        assert group * w_view * 2.0 ** qb < 2.0 ** 31
+        for v in (0, G.n_views // 3, G.n_views - 1):
+            Gv = G.with_views([G.angles[v]])
+            measured = op.siddon_back(Gv, np.ones(Gv.proj_shape)).max()
+            assert measured <= w_view, (G, v, measured, w_view)
+    qb, group, w_view = binding.siddon_fixed_point_plan(syn.workload(4).geometry)
+    assert qb == 19 and group == 40                                      # paper size: all 40 views in one group (DESIGN.md)
+
+
 def test_no_cpu_fallback_without_a_device():
     """On a box without an sm_100 GPU the product path must refuse, not fall back."""
     import torch
