@@ -346,7 +346,8 @@ def main():
     roofline = dict(bound="alu", kernel=f"cbct_{dom}", achieved=achieved_tinstr, peak=peak_tinstr, unit="Tinstr/s",
                     frac=achieved_tinstr / peak_tinstr, traffic=ncu_traffic.get((dom, args.workload)),
                     traffic_unit="DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum); algorithmic HBM bytes "
-                                 "are 105e6 per launch, the kernel is not HBM bound",
+                                 "are 105e6 per launch, the kernel is not HBM bound; taken from the committed r1 captures (scalar streams, "
+                                 "16x2 scatter layout) -- the packed default kernels move the same data and are to be re-captured",
                     algorithmic=f"{geom.n_samples} samples x {INSTR_PER_SAMPLE:.0f} thread-instr/sample per launch",
                     launch_ms=dom_ms, gsamples_s=geom.n_samples / (dom_ms * 1e-3) / 1e9,
                     peak_source=f"148 SM x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)",
