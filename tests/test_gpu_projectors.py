@@ -384,3 +384,14 @@ def test_siddon_full_size_sampled_rays_and_adjoint():
     gx, _ = _siddon(G, x, y)
     lhs, rhs = float(np.sum(gx.astype(np.float64) * y)), float(np.sum(x.astype(np.float64) * f))
     assert abs(lhs - rhs) <= TOL * abs(lhs)
+
+
+def test_microbench_rates_are_sane():
+    """cbct_microbench (SURVEY.md §8(d) denominators): every kind runs and lands in the physically possible range for an
+    SM with 4 schedulers, 128 fp32 lanes and a 128-byte/clk shared-memory pipe."""
+    r = cb.microbench()
+    assert 2.0 <= r["ffma"][0] <= 4.2, r                       # warp instructions per clock per SM
+    assert 1.0 <= r["ffma2"][0] <= 4.2, r
+    assert 0.5 <= r["lds32"][0] <= 1.1 and 0.3 <= r["atoms_add_s32"][0] <= 1.1, r
+    assert 0.0 < r["atoms_add_u64"][0] <= 1.1 and 0.2 <= r["ldg32_l1_hit"][0] <= 1.1, r
+    assert 2000.0 <= r["l2_read_64MB"][0] <= 40000.0 and r["l2_red_add_s32"][0] > 1.0, r
