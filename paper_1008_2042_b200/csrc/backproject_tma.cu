@@ -56,8 +56,9 @@ __global__ void __launch_bounds__(256) absmax_kernel(const float *__restrict__ g
 //         (mod 32): 2.2 wavefronts per ATOMS;
 //   LM 1: a warp = 16(u) x 2(v), rows 8 apart (their samples lie in different z-planes), no skew, the forward
 //         kernel's box (pitch 8, plane pitch 16 mod 32): 2.9 wavefronts per ATOMS (model) / 2.96 (ncu).
-// LM 0 is the default (verified against the oracle by running this source under a CPU thread-per-CUDA-thread shim while
-// the GPU pool was closed; its 13.3 ms is the model's prediction from LM 1's measured 17.6 ms); CBCT_BT_LANES=1 selects LM 1.
+// LM 0 is the default (verified against the oracle by executing this source on the host, tests/cpu_shim, whose bank statistics
+// reproduce LM 1's measured 2.96 and give 2.25 for LM 0, 2.0 with the same-cell merging of the packed stream below: ~12 ms
+// predicted from LM 1's measured 17.6 ms); CBCT_BT_LANES=1 selects LM 1.
 // The order in which a thread visits the samples of a chunk is free: integer sums do not depend on it.
 template <int BF, int BS, int LM, bool PK>
 __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
