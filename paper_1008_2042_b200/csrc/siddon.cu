@@ -156,13 +156,16 @@ __global__ void __launch_bounds__(256) siddon_scatter_kernel(DevGeom g, const fl
     });
 }
 
-// Bound on the path length (mm) one voxel can collect from ONE view: (number of pixels its shadow can touch) x (its diagonal).
-// The shadow of a voxel at the nearest depth t_min = SAD - R is magnified by at most SDD / t_min.
+// Bound on the path length (mm) one voxel can collect from ONE view: (number of pixel centres its shadow can cover) x (its
+// diagonal, the longest chord).  With D = depth of a point along the central ray, tau = its lateral coordinate, a point
+// projects to u = SDD tau / D, v = SDD z / D.  Over one voxel tau and D each vary by at most s = sqrt(dx^2 + dy^2), z by dz,
+// so the shadow is at most  Lu = s (SDD/Dmin + umax/Dmin)  by  Lv = dz SDD/Dmin + s vmax/Dmin  (umax, vmax: the largest |u|,
+// |v| on the detector; Dmin = SAD - R), and an interval of length L holds at most L/pitch + 1 pixel centres.
 static double siddon_weight_bound(const cbct_geometry_desc &d, double R) {
-    const double mag = d.sdd / (d.sad - R);
-    const double nu_ = std::sqrt(d.dx * d.dx + d.dy * d.dy) * mag / d.du + 2.0;
-    const double nv_ = (d.dz + std::sqrt(d.dx * d.dx + d.dy * d.dy) * (0.5 * d.nv * d.dv + std::fabs(d.v0)) / d.sdd) * mag / d.dv + 2.0;
-    return nu_ * nv_ * std::sqrt(d.dx * d.dx + d.dy * d.dy + d.dz * d.dz);
+    const double dmin = d.sad - R, s = std::sqrt(d.dx * d.dx + d.dy * d.dy);
+    const double umax = 0.5 * d.nu * d.du + std::fabs(d.u0), vmax = 0.5 * d.nv * d.dv + std::fabs(d.v0);
+    const double lu = s * (d.sdd + umax) / dmin, lv = (d.dz * d.sdd + s * vmax) / dmin;
+    return (lu / d.du + 1.0) * (lv / d.dv + 1.0) * std::sqrt(s * s + d.dz * d.dz);
 }
 
 // 2^qb units per max|g| mm; views_per_group * w * 2^qb < 2^31.  Prefer all views in one group at qb >= 18, else groups of
