@@ -147,6 +147,7 @@ struct Worker {
 static thread_local Worker *tw = nullptr;
 static const size_t STACK_BYTES = 256 * 1024, DYN_MAX = 232448;       // 227 KiB
 static const unsigned DYN_VADDR = 0x100000;
+static bool g_reverse = false;                         // SHIM_ORDER=reverse: fibers are resumed from the highest thread index down
 static bool g_lazy = false;                            // SHIM_TMA=lazy: async copies land at the last legal moment
 
 // Workers are pooled: OpenMP may retire and re-create its threads between launches, so a worker (fiber stacks,
@@ -419,7 +420,8 @@ static void run_block(Worker *w, const std::function<void()> &body, dim3 grid, d
     int idle_passes = 0;
     while (w->live > 0 && !w->aborted && !g_failed) {
         w->progress = false;
-        for (int i = 0; i < n && !w->aborted; ++i) {
+        for (int k = 0; k < n && !w->aborted; ++k) {
+            const int i = g_reverse ? n - 1 - k : k;         // SHIM_ORDER=reverse: the last thread of the block runs first
             Fiber &f = w->fibers[i];
             if (f.state != READY && f.state != SPIN) continue;
             const bool was_spin = f.state == SPIN;
@@ -461,6 +463,8 @@ void launch(const void *func, dim3 grid, dim3 block, size_t smem, const std::fun
     log_kernel(func, grid, block, smem);
     const char *mode = getenv("SHIM_TMA");
     g_lazy = mode && !strcmp(mode, "lazy");
+    const char *order = getenv("SHIM_ORDER");
+    g_reverse = order && !strcmp(order, "reverse");
     const size_t nthreads = (size_t)block.x * block.y * block.z;
     if (!nthreads || nthreads > 1024 || block.z > 64) { record_error("launch: invalid block size"); return; }
     if (!grid.x || !grid.y || !grid.z || grid.y > 65535 || grid.z > 65535) { record_error("launch: invalid grid size (y, z <= 65535)"); return; }

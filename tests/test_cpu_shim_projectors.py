@@ -82,6 +82,20 @@ def test_forward_tma_packed_and_scalar_streams_are_bit_identical(monkeypatch):
     assert rel_l2_per_view(out["1"], op.forward(RAGGED_TMA, f.astype(np.float64))) <= TOL
 
 
+@pytest.mark.parametrize("tma_mode", ["eager", "lazy"])
+def test_tma_kernels_with_reversed_thread_order(monkeypatch, tma_mode):
+    """The shim normally resumes thread 0 of a block first, which would hide a consumer running ahead of the thread that
+    plans the chunks and issues the TMA operations; here the highest thread index runs first."""
+    monkeypatch.setenv("SHIM_ORDER", "reverse")
+    monkeypatch.setenv("SHIM_TMA", tma_mode)
+    x, y = syn.uniform_volume(RAGGED_TMA, 74), syn.uniform_projections(RAGGED_TMA, 75) - 0.4
+    g, f = forward(RAGGED_TMA, x), back(RAGGED_TMA, y)
+    log = sl.kernel_log()
+    assert any(k.startswith("cbct::forward_tma_kernel<") for k in log) and any(k.startswith("cbct::backproject_scatter_kernel<") for k in log)
+    assert rel_l2_per_view(g, op.forward(RAGGED_TMA, x.astype(np.float64))) <= TOL
+    assert rel_l2(f, op.back_scatter(RAGGED_TMA, y.astype(np.float64))) <= TOL
+
+
 def test_forward_fallback_kernels(monkeypatch):
     f = syn.uniform_volume(ODD, 23)
     ref = op.forward(ODD, f.astype(np.float64))
