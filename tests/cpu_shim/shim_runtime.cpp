@@ -147,7 +147,7 @@ struct Worker {
 static thread_local Worker *tw = nullptr;
 static const size_t STACK_BYTES = 256 * 1024, DYN_MAX = 232448;       // 227 KiB
 static const unsigned DYN_VADDR = 0x100000;
-static bool g_reverse = false;                         // SHIM_ORDER=reverse: fibers are resumed from the highest thread index down
+static int g_order = 0;                                // SHIM_ORDER: 0 ascending, 1 reverse, 2 random (seeded per block)
 static bool g_lazy = false;                            // SHIM_TMA=lazy: async copies land at the last legal moment
 
 // Workers are pooled: OpenMP may retire and re-create its threads between launches, so a worker (fiber stacks,
@@ -418,10 +418,14 @@ static void run_block(Worker *w, const std::function<void()> &body, dim3 grid, d
         makecontext(&f.ctx, fiber_entry, 0);
     }
     int idle_passes = 0;
+    unsigned long long rng = 0x9e3779b97f4a7c15ull ^ ((unsigned long long)bid.x << 40) ^ ((unsigned long long)bid.y << 20) ^ bid.z;
     while (w->live > 0 && !w->aborted && !g_failed) {
         w->progress = false;
+        rng = rng * 6364136223846793005ull + 1442695040888963407ull;
+        const unsigned rot = (unsigned)(rng >> 33) % (unsigned)n, rdir = (unsigned)(rng >> 20) & 1u;
         for (int k = 0; k < n && !w->aborted; ++k) {
-            const int i = g_reverse ? n - 1 - k : k;         // SHIM_ORDER=reverse: the last thread of the block runs first
+            // SHIM_ORDER=reverse: the last thread of the block runs first; random: a different rotation and direction per pass
+            const int i = g_order == 1 ? n - 1 - k : (g_order == 2 ? (int)((rot + (unsigned)(rdir ? k : n - 1 - k)) % (unsigned)n) : k);
             Fiber &f = w->fibers[i];
             if (f.state != READY && f.state != SPIN) continue;
             const bool was_spin = f.state == SPIN;
@@ -464,7 +468,7 @@ void launch(const void *func, dim3 grid, dim3 block, size_t smem, const std::fun
     const char *mode = getenv("SHIM_TMA");
     g_lazy = mode && !strcmp(mode, "lazy");
     const char *order = getenv("SHIM_ORDER");
-    g_reverse = order && !strcmp(order, "reverse");
+    g_order = !order ? 0 : (!strcmp(order, "reverse") ? 1 : (!strcmp(order, "random") ? 2 : 0));
     const size_t nthreads = (size_t)block.x * block.y * block.z;
     if (!nthreads || nthreads > 1024 || block.z > 64) { record_error("launch: invalid block size"); return; }
     if (!grid.x || !grid.y || !grid.z || grid.y > 65535 || grid.z > 65535) { record_error("launch: invalid grid size (y, z <= 65535)"); return; }

@@ -82,11 +82,13 @@ def test_forward_tma_packed_and_scalar_streams_are_bit_identical(monkeypatch):
     assert rel_l2_per_view(out["1"], op.forward(RAGGED_TMA, f.astype(np.float64))) <= TOL
 
 
+@pytest.mark.parametrize("order", ["reverse", "random"])
 @pytest.mark.parametrize("tma_mode", ["eager", "lazy"])
-def test_tma_kernels_with_reversed_thread_order(monkeypatch, tma_mode):
+def test_tma_kernels_with_other_thread_orders(monkeypatch, tma_mode, order):
     """The shim normally resumes thread 0 of a block first, which would hide a consumer running ahead of the thread that
-    plans the chunks and issues the TMA operations; here the highest thread index runs first."""
-    monkeypatch.setenv("SHIM_ORDER", "reverse")
+    plans the chunks and issues the TMA operations; here the highest thread index runs first, or the order changes
+    (rotation and direction, seeded per block) between every two scheduling points."""
+    monkeypatch.setenv("SHIM_ORDER", order)
     monkeypatch.setenv("SHIM_TMA", tma_mode)
     x, y = syn.uniform_volume(RAGGED_TMA, 74), syn.uniform_projections(RAGGED_TMA, 75) - 0.4
     g, f = forward(RAGGED_TMA, x), back(RAGGED_TMA, y)
