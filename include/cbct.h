@@ -15,9 +15,23 @@
  *     as void* (NULL = the legacy default stream).
  *   - in and out must not alias unless a function says "in place".  Outputs are overwritten.
  *   - Hot calls are asynchronous on `stream`, allocate nothing and never synchronise the host; they
- *     return launch errors only.  Handles own their device workspace (allocated at *_create).
- *   - Return value: 0 = CBCT_OK, < 0 = error, CBCT_BREAKDOWN (+1) = CGLS breakdown (not a failure).
+ *     return launch errors only.  Handles own their device workspace (allocated at *_create / *_prepare).
+ *   - A handle's workspace is used by every call on it: ONE call in flight per handle (calls on the same
+ *     stream are ordered and therefore fine; two streams or threads sharing a handle are not).
+ *   - Return value: 0 = CBCT_OK, < 0 = error, CBCT_BREAKDOWN (+1) = CGLS breakdown (not a failure;
+ *     SURVEY.md §8(b) calls it CBCT_E_BREAKDOWN, the E_ is dropped here because it is not an error).
  *     Nothing throws or aborts.
+ *   - No kernel of this library waits without a bound or indexes shared memory unchecked: a TMA copy that never
+ *     arrives, or a sampling box that does not cover its samples, raises the handle's device error word
+ *     (cbct_geometry_status) and the kernel leaves through its normal exit path; every later call on the handle
+ *     returns CBCT_E_DEVICE until the word is cleared.
+ *   - Which kernel variant serves a handle is decided once, in cbct_geometry_create (cbct_geometry_describe reports
+ *     it).  The selection variables below are read THERE and nowhere else; they exist for tests and A/B timing:
+ *       CBCT_FORWARD_IMPL = tma | tiled | global      CBCT_BACKPROJECT_IMPL = scatter | cell | gather
+ *       CBCT_FW_PACKED = 0|1   CBCT_BT_PACKED = 0|1   (packed fp32-pair or scalar instruction stream)
+ *       CBCT_BT_LANES = 0|1    (lane layout of the scatter kernel)
+ *     A forced implementation that the geometry cannot use makes cbct_geometry_create fail (CBCT_E_UNSUPPORTED);
+ *     nothing falls back silently at launch time.
  */
 #ifndef CBCT_H
 #define CBCT_H
@@ -34,7 +48,14 @@ enum {
     CBCT_E_INVALID = -1,      /* bad argument (null pointer, non-positive size, geometry rejected) */
     CBCT_E_UNSUPPORTED = -2,  /* no sm_100-class device / feature not available */
     CBCT_E_CUDA = -3,         /* a CUDA runtime call failed; see cbct_last_cuda_error() */
+    CBCT_E_DEVICE = -4,       /* a kernel raised the handle's device error word; see cbct_geometry_status() */
     CBCT_BREAKDOWN = 1        /* CGLS: gamma == 0 or ||q||^2 == 0 (PAPER.md:446, :461 would divide by 0) */
+};
+/* bits of the device error word (cbct_geometry_status) */
+enum {
+    CBCT_STATUS_WAIT_TIMEOUT = 1,       /* a bounded mbarrier wait expired (TMA copy never completed) */
+    CBCT_STATUS_FORWARD_RANGE = 2,      /* cbct_forward: a thread's samples left the staged box (skipped, not read) */
+    CBCT_STATUS_BACKPROJECT_RANGE = 4   /* cbct_backproject: a thread's samples left the accumulator box (skipped) */
 };
 
 /* Static string for a status code. */
@@ -43,13 +64,7 @@ const char *cbct_status_string(int status);
 int cbct_last_cuda_error(void);
 /* Library version, e.g. 100 = 1.0.0. */
 int cbct_version(void);
-/* Number of kernels of this library launched by this process so far (all threads). */
-long long cbct_launch_count(void);
-/* Optional kernel timer.  Between _begin and _end every cbct_forward / cbct_backproject launch (also
- * those inside CGLS and the driver) is bracketed by CUDA events on its own stream.  _end waits for
- * those events and returns the summed device time in ms and the launch count, index 0 = P, 1 = P^T. */
-int cbct_profile_begin(void);
-int cbct_profile_end(double ms[2], int count[2]);
+/* (Probes -- launch counter, kernel timer, micro-benchmarks -- are declared in cbct_debug.h.) */
 
 /* ------------------------------------------------------------------------------------------------
  * Geometry: circular orbit, flat panel (Eq. 1, Fig. 1 caption).
@@ -89,6 +104,16 @@ int cbct_geometry_info(const cbct_geometry *geom, int64_t *n_vox, int64_t *n_ray
                        double *t_min, double *step_mm, int64_t *n_samples_algorithmic,
                        size_t *workspace_bytes);
 
+/* The kernels that serve this handle, as text, e.g.
+ *   "forward: forward_tma_kernel<40,30,scalar> box 40x30x7; backproject: backproject_scatter_kernel<40,30,LM1,scalar> ..."
+ * written to buf (NUL-terminated, truncated to cap).  Host only. */
+int cbct_geometry_describe(const cbct_geometry *geom, char *buf, size_t cap);
+
+/* Device error word of the handle.  Synchronises `stream`, stores the CBCT_STATUS_* bits raised by kernels of this
+ * handle since the last clear in *flags (may be NULL), clears the word if `clear` != 0.
+ * Returns CBCT_OK if no bit was set, CBCT_E_DEVICE otherwise. */
+int cbct_geometry_status(cbct_geometry *geom, void *stream, int *flags, int clear);
+
 /* g = P f.  PAPER.md:73 Eq. 1 discretised as step * sum_k T[f](x_S + n t_k), T = zero-padded
  * trilinear interpolation (north_star).  d_vol: nx*ny*nz, d_proj: n_views*nv*nu. */
 int cbct_forward(const cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
@@ -113,27 +138,19 @@ int cbct_backproject_eq3(const cbct_geometry *geom, const float *d_proj, float *
  * segment from the source to the pixel centre.  No sampling step: geom's step_mm is not used.  A second matched pair
  * next to cbct_forward / cbct_backproject (which are the fixed-step trilinear pair north_star prescribes); CGLS in this
  * library uses the trilinear pair.  Buffers and conventions as cbct_forward / cbct_backproject; outputs overwritten.
- * The handle is not const: the first call allocates the pair's workspace (a y-fastest volume copy; for the transpose
- * two int32 accumulator volumes) with cudaMalloc, i.e. the FIRST call synchronises the device; later calls are
- * asynchronous on `stream`.  cbct_siddon_backproject accumulates in fixed point relative to max|g| (deterministic,
+ * cbct_siddon_prepare allocates the pair's workspace (a y-fastest volume copy, two int32 accumulator volumes; synchronous)
+ * and must be called once per handle before the two hot calls, which return CBCT_E_INVALID otherwise and, like every hot
+ * call, allocate nothing.  cbct_siddon_backproject accumulates in fixed point relative to max|g| (deterministic,
  * error per contribution <= max|g| / 2^(qb+1) mm with qb >= 9 chosen from a bound on the path length one voxel can
  * collect); CBCT_E_UNSUPPORTED if no qb satisfies the bound. */
-int cbct_siddon_forward(cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
-int cbct_siddon_backproject(cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
+int cbct_siddon_prepare(cbct_geometry *geom);
+int cbct_siddon_forward(const cbct_geometry *geom, const float *d_vol, float *d_proj, void *stream);
+int cbct_siddon_backproject(const cbct_geometry *geom, const float *d_proj, float *d_vol, void *stream);
 
 /* Host arithmetic only: the fixed-point plan of cbct_siddon_backproject.  max_path_sum_per_view bounds the path length
  * (mm) one voxel can collect from one view: (pixels its shadow can touch at the nearest depth) x (voxel diagonal);
  * views_per_group * max_path_sum_per_view * 2^qb < 2^31.  CBCT_E_UNSUPPORTED if no qb >= 9 fits one view. */
 int cbct_siddon_fixed_point_plan(const cbct_geometry_desc *desc, int32_t *qb, int32_t *views_per_group, double *max_path_sum_per_view);
-
-/* Micro-benchmarks of the per-SM rates that bound the projector kernels on the device in use (the
- * denominators MEASURED_PEAKS.json does not have).  Synchronises `stream`.  kind:
- *   0 FFMA, 1 FFMA2 (packed pair), 2 LDS.32 conflict-free, 3 ATOMS.ADD.S32 conflict-free, 4 LDG.32 hitting L1
- *     -> out[0] = warp instructions per clock per SM (clock64 inside the kernel, slowest warp of 32 per SM);
- *   7 ATOMS.ADD.64 conflict-free (256 contiguous bytes per instruction) -> warp instructions per clock per SM;
- *   5 L2 read bandwidth on a 64 MB set -> out[0] = GB/s;   6 coalesced RED.ADD.S32 into a 64 MB set -> out[0] = 1e9 reductions/s.
- * out[1] = seconds of the measured launch (CUDA events), out[2] = its work items. */
-int cbct_microbench(int kind, double out[3], void *stream);
 
 /* Host arithmetic only (no device needed): the fixed-point plan cbct_backproject uses for this geometry.
  *   max_weight_sum_per_view: upper bound on the sum of trilinear weights one voxel receives from one view;
@@ -169,7 +186,8 @@ int cbct_cgls_init(cbct_cgls *cg, const float *d_g, const float *d_x, float *d_r
 int cbct_cgls_step(cbct_cgls *cg, float *d_x, float *d_r, float *d_p, void *stream);
 
 /* Synchronises `stream` and copies out {gamma, ||q||^2, alpha, beta, ||r||^2}.  ||r||^2 is computed
- * here from d_r if d_r != NULL, else reported as -1.  Returns CBCT_BREAKDOWN if the flag is set. */
+ * here from d_r if d_r != NULL, else reported as -1 (the residual belongs to the caller, so it is an
+ * argument here; SURVEY.md §8(b) sketched the call without it).  Returns CBCT_BREAKDOWN if the flag is set. */
 int cbct_cgls_scalars(cbct_cgls *cg, const float *d_r, double out[5], void *stream);
 
 /* ------------------------------------------------------------------------------------------------

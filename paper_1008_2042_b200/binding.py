@@ -15,15 +15,17 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcbct_b200.so")
 
-CBCT_OK, CBCT_E_INVALID, CBCT_E_UNSUPPORTED, CBCT_E_CUDA, CBCT_BREAKDOWN = 0, -1, -2, -3, 1
+CBCT_OK, CBCT_E_INVALID, CBCT_E_UNSUPPORTED, CBCT_E_CUDA, CBCT_E_DEVICE, CBCT_BREAKDOWN = 0, -1, -2, -3, -4, 1
+STATUS_BITS = {1: "wait_timeout", 2: "forward_range", 4: "backproject_range"}
 
-# every symbol include/cbct.h declares (tests check the library exports all of them)
+# every symbol include/cbct.h and include/cbct_debug.h declare (tests check the library exports all of them)
 EXPORTS = [
     "cbct_status_string", "cbct_last_cuda_error", "cbct_version", "cbct_launch_count",
     "cbct_profile_begin", "cbct_profile_end",
-    "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info",
+    "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_info", "cbct_geometry_describe", "cbct_geometry_status",
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
-    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_forward", "cbct_siddon_backproject", "cbct_siddon_fixed_point_plan", "cbct_microbench",
+    "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_prepare", "cbct_siddon_forward", "cbct_siddon_backproject",
+    "cbct_siddon_fixed_point_plan", "cbct_microbench", "tf_reconstruct_direct",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
@@ -81,12 +83,15 @@ def _declare(L):
     L.cbct_geometry_info.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64),
                                      C.POINTER(C.c_size_t)]
+    L.cbct_geometry_describe.argtypes = [vp, C.c_char_p, C.c_size_t]
+    L.cbct_geometry_status.argtypes = [vp, vp, C.POINTER(C.c_int), ip]
+    L.cbct_siddon_prepare.argtypes = [vp]
     for name in ("cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host", "cbct_backproject_eq3",
                  "cbct_siddon_forward", "cbct_siddon_backproject"):
         getattr(L, name).argtypes = [vp, fp, fp, vp]
     L.cbct_siddon_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                                C.POINTER(C.c_double)]
-    L.cbct_microbench.argtypes = [ip, C.POINTER(C.c_double), vp]
+    L.cbct_microbench.argtypes = [ip, ip, C.POINTER(C.c_double), vp]
     L.cbct_backproject_fixed_point_plan.argtypes = [C.POINTER(GeometryDesc), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                                     C.POINTER(C.c_double)]
     L.cbct_cgls_create.argtypes = [vp, C.POINTER(vp)]
@@ -97,6 +102,7 @@ def _declare(L):
     L.tf_decompose.argtypes = [fp, fp, ip, ip, ip, vp]
     L.tf_shrink.argtypes = [fp, C.c_float, ip, ip, ip, vp]
     L.tf_reconstruct.argtypes = [fp, fp, ip, ip, ip, vp]
+    L.tf_reconstruct_direct.argtypes = [fp, fp, ip, ip, ip, vp]
     L.tf_apply_fused.argtypes = [fp, fp, C.c_float, ip, ip, ip, ip, vp]
     L.mg_restrict.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
     L.mg_prolong.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
@@ -182,12 +188,12 @@ MICROBENCH_KINDS = {0: ("ffma", "warp-instr/clk/SM"), 1: ("ffma2", "warp-instr/c
                     5: ("l2_read_64MB", "GB/s"), 6: ("l2_red_add_s32", "Gred/s"), 7: ("atoms_add_u64", "warp-instr/clk/SM")}
 
 
-def microbench(stream=None):
-    """{name: (rate, unit)} of cbct_microbench for every kind."""
+def microbench(stream=None, iters: int = 0):
+    """{name: (rate, unit)} of cbct_microbench for every kind; iters <= 0: the default loop length."""
     res = {}
     for kind, (name, unit) in MICROBENCH_KINDS.items():
         out = (C.c_double * 3)()
-        _check(lib().cbct_microbench(kind, out, _stream(stream)), "cbct_microbench")
+        _check(lib().cbct_microbench(kind, int(iters), out, _stream(stream)), "cbct_microbench")
         res[name] = (out[0], unit)
     return res
 
@@ -226,11 +232,31 @@ class Geometry:
         self.t_min, self.step_mm, self.n_samples, self.workspace_bytes = t0.value, st.value, ns.value, ws.value
         self.vol_shape = (geom.nz, geom.ny, geom.nx)
         self.proj_shape = (len(tuple(geom.angles)), geom.nv, geom.nu)
+        self._siddon_ready = False
 
     def close(self):
         if getattr(self, "handle", None):
             lib().cbct_geometry_destroy(self.handle)
             self.handle = None
+
+    def describe(self) -> str:
+        """which kernels serve this handle (cbct_geometry_describe)"""
+        buf = C.create_string_buffer(512)
+        _check(lib().cbct_geometry_describe(self.handle, buf, len(buf)), "cbct_geometry_describe")
+        return buf.value.decode()
+
+    def status(self, clear: bool = False, stream=None):
+        """(ok, [names of the raised CBCT_STATUS_* bits]); synchronises the stream (cbct_geometry_status)"""
+        flags = C.c_int(0)
+        s = lib().cbct_geometry_status(self.handle, _stream(stream), C.byref(flags), int(clear))
+        if s not in (CBCT_OK, CBCT_E_DEVICE):
+            raise CbctError(s, "cbct_geometry_status")
+        return s == CBCT_OK, [n for b, n in STATUS_BITS.items() if flags.value & b]
+
+    def siddon_prepare(self):
+        if not self._siddon_ready:
+            _check(lib().cbct_siddon_prepare(self.handle), "cbct_siddon_prepare")
+            self._siddon_ready = True
 
     def __del__(self):
         try:
@@ -256,12 +282,14 @@ class Geometry:
 
     def siddon_forward(self, d_vol, d_proj, stream=None):
         """g = P_siddon f: the paper's own projector, exact path lengths through piecewise-constant voxels."""
+        self.siddon_prepare()
         _check(lib().cbct_siddon_forward(self.handle, _dptr(d_vol, self.n_vox), _dptr(d_proj, self.n_rays), _stream(stream)),
                "cbct_siddon_forward")
         return d_proj
 
     def siddon_backproject(self, d_proj, d_vol, stream=None):
         """f = P_siddon^T g, the exact transpose of siddon_forward."""
+        self.siddon_prepare()
         _check(lib().cbct_siddon_backproject(self.handle, _dptr(d_proj, self.n_rays), _dptr(d_vol, self.n_vox), _stream(stream)),
                "cbct_siddon_backproject")
         return d_vol
@@ -336,6 +364,14 @@ def tf_reconstruct(d_alpha, d_f, stream=None):
     nx, ny, nz = _dims(d_f.shape)
     _check(lib().tf_reconstruct(_dptr(d_alpha, 27 * nx * ny * nz), _dptr(d_f), nx, ny, nz, _stream(stream)),
            "tf_reconstruct")
+    return d_f
+
+
+def tf_reconstruct_direct(d_alpha, d_f, stream=None):
+    """cbct_debug.h: the 27 x 27-tap cross-check of tf_reconstruct"""
+    nx, ny, nz = _dims(d_f.shape)
+    _check(lib().tf_reconstruct_direct(_dptr(d_alpha, 27 * nx * ny * nz), _dptr(d_f), nx, ny, nz, _stream(stream)),
+           "tf_reconstruct_direct")
     return d_f
 
 

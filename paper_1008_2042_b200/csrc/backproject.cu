@@ -288,6 +288,7 @@ static double nudge(double a, double floor_mag) {
 }
 
 int build_bp_tables(cbct_geometry *G) {
+    if (G->bp_impl != BP_CELL) return CBCT_OK;        // tables and partial volumes of a kernel that will not run
     const cbct_geometry_desc &d = G->desc;
     const int nu = d.nu, nv = d.nv, nvw = d.n_views;
     std::vector<BpView> views(nvw);
@@ -335,8 +336,9 @@ int build_bp_tables(cbct_geometry *G) {
     if (e == cudaSuccess) e = cudaMalloc((void **)&T.viewu, sizeof(BpViewU) * viewu.size());
     if (e == cudaSuccess) e = cudaMalloc((void **)&T.pixT, sizeof(float4) * pix.size());
     if (e == cudaSuccess) e = cudaMalloc((void **)&T.rows, sizeof(float2) * rows.size());
-    if (e == cudaSuccess) e = cudaMalloc((void **)&G->d_bp_partial, sizeof(float) * 8 * ncell);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&G->d_bp_projT, sizeof(float) * G->n_rays);
+    const bool cell = true;
+    if (e == cudaSuccess && cell) e = cudaMalloc((void **)&G->d_bp_partial, sizeof(float) * 8 * ncell);
+    if (e == cudaSuccess && cell) e = cudaMalloc((void **)&G->d_bp_projT, sizeof(float) * G->n_rays);
     if (e == cudaSuccess) e = cudaMemcpy((void *)T.views, views.data(), sizeof(BpView) * views.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy((void *)T.viewu, viewu.data(), sizeof(BpViewU) * viewu.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy((void *)T.pixT, pix.data(), sizeof(float4) * pix.size(), cudaMemcpyHostToDevice);
@@ -349,19 +351,18 @@ int build_bp_tables(cbct_geometry *G) {
     T.k_eps = (float)std::fmax(0.02, 4.0 * 1.2e-7 * (d.sad + G->R) / G->step);   // fp32 rounding of r*L, in samples
     T.stepf = (float)G->step; T.tau0f = (float)(G->t_min + 0.5 * G->step - d.sad);
     G->workspace_bytes += sizeof(BpView) * views.size() + sizeof(BpViewU) * viewu.size() + sizeof(float4) * pix.size() +
-                          sizeof(float2) * rows.size() + sizeof(float) * 8 * ncell + sizeof(float) * G->n_rays;
+                          sizeof(float2) * rows.size() + (cell ? sizeof(float) * 8 * ncell + sizeof(float) * G->n_rays : 0);
     return CBCT_OK;
 }
 
 int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
     const DevGeom &g = G->dg;
     ProfScope prof(PROF_BACK, st);
-    // CBCT_BACKPROJECT_IMPL = "gather" | "cell" | "scatter" forces one implementation (tests); default: scatter
-    // (backproject_tma.cu) when the geometry supports it, else the cell-driven kernel below
-    const char *impl = getenv("CBCT_BACKPROJECT_IMPL");
-    if (impl && impl[0] == 's') return launch_backproject_tma(G, d_proj, d_vol, st);
-    if (!impl && G->bt_ok) return launch_backproject_tma(G, d_proj, d_vol, st);
-    if (impl && impl[0] == 'g') {
+    CBCT_TRY(device_error_pending(G));
+    // the implementation was fixed at cbct_geometry_create (G->bp_impl): scatter (backproject_tma.cu) where the geometry
+    // supports it, else the cell-driven kernel below; gather = the per-voxel cross-check
+    if (G->bp_impl == BP_SCATTER) return launch_backproject_tma(G, d_proj, d_vol, st);
+    if (G->bp_impl == BP_GATHER) {
         dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4), g.nz);
         backproject_gather_kernel<<<grid, block, 0, st>>>(g, d_proj, d_vol);
         CBCT_LAUNCH_CHECK();
@@ -376,8 +377,7 @@ int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol
         // block = xb x-neighbouring columns of nz+1 cells, lanes along z; xb minimises idle lanes
         const int nzc = g.nz + 1;
         int xb = 1, best_waste = 1 << 30;
-        const char *mt = getenv("CBCT_BP_MAXT");
-        const int max_threads = mt ? atoi(mt) : 320;
+        const int max_threads = 320;
         for (int c = 1; c <= 16 && c * nzc <= max_threads; ++c) {
             const int th = ((c * nzc + 31) / 32) * 32, waste = (th - c * nzc) * 1024 / th;
             if (th >= 128 && waste < best_waste) { best_waste = waste; xb = c; }

@@ -20,7 +20,7 @@
 // result that is ~1e-6 * max|g| / rms(g) -- an order of magnitude below the fp32 rounding of the weights
 // themselves for any input whose peak is within ~30 rms (projections, CGLS residuals).
 #include <cmath>
-#include <cstdlib>
+#include <cstdio>
 #include <cstring>
 
 #include "tma_common.cuh"
@@ -33,19 +33,23 @@ constexpr int BT_ROUND_BITS = 0x4B400000;
 // integer nearest to c = a*b (|c| < 2^22), in one FFMA + one IADD
 __device__ __forceinline__ int round_mul(float a, float b) { return __float_as_int(fmaf(a, b, BT_ROUND)) - BT_ROUND_BITS; }
 
-// max |g| as the bit pattern of a non-negative float (orders like an unsigned integer); *out zeroed before
+// max |g| as the bit pattern of a non-negative float (orders like an unsigned integer); *out zeroed before.
+// The maximum is taken on the bit patterns, so an Inf or NaN anywhere in g wins (their patterns exceed every finite
+// one): the scatter kernels then contribute nothing and the finalize pass multiplies by a non-finite factor, i.e. a
+// non-finite input gives an all-NaN volume instead of finite garbage.
 __global__ void __launch_bounds__(256) absmax_kernel(const float *__restrict__ g, long long n, unsigned *out) {
-    float m = 0.f;
-    const long long n4 = n >> 2;
+    unsigned m = 0u;
+    const bool vec = (reinterpret_cast<uintptr_t>(g) & 15) == 0;          // float4 loads only from a 16-byte aligned base
+    const long long n4 = vec ? n >> 2 : 0;
     const float4 *g4 = reinterpret_cast<const float4 *>(g);
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) {
         const float4 v = __ldg(g4 + i);
-        m = fmaxf(m, fmaxf(fmaxf(fabsf(v.x), fabsf(v.y)), fmaxf(fabsf(v.z), fabsf(v.w))));
+        m = max(max(m, __float_as_uint(fabsf(v.x))), max(__float_as_uint(fabsf(v.y)), max(__float_as_uint(fabsf(v.z)), __float_as_uint(fabsf(v.w)))));
     }
-    if (blockIdx.x == 0 && threadIdx.x < (n & 3)) m = fmaxf(m, fabsf(__ldg(g + (n4 << 2) + threadIdx.x)));
-    unsigned b = __float_as_uint(m);
-    b = __reduce_max_sync(0xffffffffu, b);
-    if ((threadIdx.x & 31) == 0 && b) atomicMax(out, b);
+    for (long long i = (n4 << 2) + blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        m = max(m, __float_as_uint(fabsf(__ldg(g + i))));
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
 }
 
 // Bank conflicts decide the speed of this kernel (it is bound by shared-memory wavefronts: two lanes of one
@@ -65,13 +69,13 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
                                                                          const __grid_constant__ CUtensorMap map_y,
                                                                          const float *__restrict__ proj, int *__restrict__ acc_x,
                                                                          const unsigned *__restrict__ absmax_bits, float two_qb,
-                                                                         int view0, float margin, int bzz, int dbg) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
+                                                                         int view0, float margin, int bzz, DevErr err) {
+    extern __shared__ unsigned char smem_raw[];
     __shared__ RayL corner[4];
     __shared__ ChunkPlan plans[2];
-    __shared__ int s_klo, s_khi;
+    __shared__ int s_klo, s_khi, s_abort;
     constexpr int bfs = BF, bss = BS;
-    int *buf0 = reinterpret_cast<int *>(smem_raw);
+    int *buf0 = reinterpret_cast<int *>(align128(smem_raw));      // the launch reserves 128 bytes for this
     const int box_words = bfs * bss * bzz;
     const int box_elems = (box_words + 31) & ~31;          // buffer stride: keeps the second buffer 128-byte aligned
 
@@ -114,10 +118,10 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
 
     // ray value in fixed-point units: |gs| <= 2^qb
     const float amax = __uint_as_float(__ldg(absmax_bits));
-    const float scale = amax > 0.f ? two_qb / amax : 0.f;
+    const float scale = (amax > 0.f && amax <= 3.0e38f) ? two_qb / amax : 0.f;      // non-finite max|g|: contribute nothing (finalize writes NaN)
     const float gs = valid ? __ldg(proj + ((size_t)view * g.nv + iv) * g.nu + iu) * scale : 0.f;
 
-    if (tid == 0) { s_klo = 0x7fffffff; s_khi = -1; }
+    if (tid == 0) { s_klo = 0x7fffffff; s_khi = -1; s_abort = *reinterpret_cast<volatile int *>(err.dev); }
     if ((tu == 0 || tu == FT_TU - 1) && (tv == 0 || tv == FT_TV - 1)) corner[(tv ? 2 : 0) + (tu ? 1 : 0)] = rl;
     {   // both accumulator boxes start at zero
         int4 *z = reinterpret_cast<int4 *>(buf0);
@@ -130,7 +134,7 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
     }
     __syncthreads();
     const int K0 = s_klo, K1 = s_khi;
-    if (K0 > K1) return;
+    if (K0 > K1 || s_abort) return;                           // nothing to do / an earlier CTA or call already failed
     const float stepf = (float)g.step;
     const float sF = rl.bf * stepf, sS = rl.bs * stepf, sZ = rl.bz * stepf;
     constexpr int pS = BF, pZ = BF * BS;
@@ -145,7 +149,7 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
         if (tid == 0 && kn <= K1) plans[stage ^ 1] = plan_chunk(g, corner, kn, K1, margin, bfs, bss, bzz);
         const int ja = max(k0, klo), jb = min(kn - 1, khi);
         if (cur.box.fits) {
-            if (ja <= jb && !(dbg & 2)) {
+            if (ja <= jb) {
                 const float tau_a = fmaf((float)(ja - k0), stepf, cur.tau_base);
                 const float F0 = fmaf(rl.bf, tau_a, rl.cf - (float)cur.box.lf);
                 const float S0 = fmaf(rl.bs, tau_a, rl.cs - (float)cur.box.ls);
@@ -153,7 +157,9 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
                 const unsigned base_r = smem_u32(buf0 + stage * box_elems);
                 const float pSf = (float)pS, pZf = (float)pZ;
                 const int n = jb - ja + 1;
-                if constexpr (PK) {
+                if (!(run_inside(F0, sF, n, bfs) && run_inside(S0, sS, n, bss) && run_inside(Z0, sZ, n, bzz))) {
+                    raise_device_error(err, DEV_ERR_BT_RANGE);          // never index outside the box: skip, report
+                } else if constexpr (PK) {
                     // Packed pairs (FFMA2 / FADD2 / FMUL2), two consecutive samples per pair, as in forward_tma_kernel: the
                     // positions, floors and fractions are bit-identical to the forward kernel's.  The thread starts `skew`
                     // samples ahead (kept even, so pairs never straddle the wrap-around) and visits [s0, n) then [0, s0).
@@ -267,7 +273,7 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
         }
         if (tid == 0) bulk_wait_read0();                  // the other box's reduction (issued one chunk ago) has read it
         __syncthreads();                                  // A: everyone finished scattering into box `stage`
-        if (tid == 0 && cur.box.fits && !(dbg & 1)) {
+        if (tid == 0 && cur.box.fits) {
             // The accumulator volumes carry a low-side margin of one box (a tensor reduction may not start at a
             // negative coordinate; elements beyond the high side are skipped by the TMA unit).  A box that starts
             // below the margin, or beyond the high side, lies entirely outside the volume: nothing to add.
@@ -320,12 +326,9 @@ __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__
 }
 
 typedef void (*ScatterKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, int *, const unsigned *, float, int,
-                              float, int, int);
-// CBCT_BT_PACKED=0 selects the scalar instruction stream of the scatter kernel; default: packed pairs
-static bool scatter_packed() {
-    const char *e = getenv("CBCT_BT_PACKED");
-    return !(e && atoi(e) == 0);
-}
+                              float, int, DevErr);
+// two accumulator boxes (each a multiple of 128 bytes) + 128 bytes for the in-kernel alignment of the base
+static size_t bt_smem_bytes(int bf, int bs, int bz) { return (size_t)2 * ((bf * bs * bz + 31) & ~31) * 4 + 128; }
 static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm, bool pk) {
 #define CBCT_SK(F, S, L) \
     if (bf == F && bs == S && lm == L) return pk ? backproject_scatter_kernel<F, S, L, true> : backproject_scatter_kernel<F, S, L, false>;
@@ -372,12 +375,10 @@ void plan_backproject_tma(cbct_geometry *G) {
     const cbct_geometry_desc &d = G->desc;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
     if (!G->fw_tma_ok) return;
-    // lane layout (see the kernel): default 0 = the skewed 8x4 layout, whose box is the forward kernel's with the row
-    // count rounded up to a multiple of 4 (plane pitch = 0 mod 32); CBCT_BT_LANES=1 selects 16x2 with forward's box
-    const char *lm_env = getenv("CBCT_BT_LANES");
-    G->bt_lm = (lm_env && atoi(lm_env) == 1) ? 1 : 0;
+    // lane layout G->bt_lm (see the kernel; chosen by cbct_geometry_create): 0 = the skewed 8x4 layout, whose box is the
+    // forward kernel's with the row count rounded up to a multiple of 4 (plane pitch = 0 mod 32); 1 = 16x2, forward's box
     G->bt_b = G->fw_b; G->bt_bz = G->fw_bz; G->bt_bs = G->bt_lm == 0 ? (G->fw_bs + 3) & ~3 : G->fw_bs;
-    if ((size_t)2 * G->bt_b * G->bt_bs * G->bt_bz * 4 > 100 * 1024) return;
+    if (bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz) > 101 * 1024) return;
     int qb = 0, group = 0;
     double w_view = 0;
     if (!bt_fixed_point_plan(d, G->R, G->step, &qb, &group, &w_view)) return;
@@ -405,8 +406,8 @@ void plan_backproject_tma(cbct_geometry *G) {
     std::memcpy(G->bt_map_y, &my, sizeof(my));
     for (int pk = 0; pk < 2; ++pk) {
         ScatterKernel k = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, pk != 0);
-        if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) !=
-                      cudaSuccess) {
+        if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz)) != cudaSuccess) {
             (void)cudaGetLastError();
             free_backproject_tma(G);
             return;
@@ -421,19 +422,18 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
     CUtensorMap mx, my;
     std::memcpy(&mx, G->bt_map_x, sizeof(mx));
     std::memcpy(&my, G->bt_map_y, sizeof(my));
-    ScatterKernel kern = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, scatter_packed());
+    ScatterKernel kern = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, G->bt_packed != 0);
     if (!kern) return CBCT_E_UNSUPPORTED;
     CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_absmax, 0, sizeof(unsigned), st));
     absmax_kernel<<<592, 256, 0, st>>>(d_proj, (long long)G->n_rays, G->d_bt_absmax);
     CBCT_LAUNCH_CHECK();
-    const size_t smem = (size_t)2 * ((G->bt_b * G->bt_bs * G->bt_bz + 31) & ~31) * 4;
+    const size_t smem = bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz);
     const float two_qb = (float)std::ldexp(1.0, G->bt_qb);
-    const int dbg = getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0;
     for (int v0 = 0; v0 < g.n_views; v0 += G->bt_group) {
         const int nv_ = std::min(G->bt_group, g.n_views - v0);
         CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_acc, 0, sizeof(int) * G->bt_acc_elems, st));
         dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), nv_);
-        kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_proj, G->d_bt_acc, G->d_bt_absmax, two_qb, v0, G->fw_margin, G->bt_bz, dbg);
+        kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_proj, G->d_bt_acc, G->d_bt_absmax, two_qb, v0, G->fw_margin, G->bt_bz, G->err);
         CBCT_LAUNCH_CHECK();
         dim3 fb(32, 8), fg(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
         backproject_finalize_kernel<<<fg, fb, 0, st>>>(G->d_bt_acc, G->d_bt_acc + G->bt_acc_y_off, d_vol, g.nx, g.ny, G->bt_b, G->bt_bs,
@@ -442,6 +442,11 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;
+}
+
+void describe_backproject_tma(const cbct_geometry *G, char *buf, size_t cap) {
+    snprintf(buf, cap, "backproject_scatter_kernel<%d,%d,LM%d,%s> box %dx%dx%d qb %d views/group %d", G->bt_b, G->bt_bs, G->bt_lm,
+             G->bt_packed ? "packed" : "scalar", G->bt_b, G->bt_bs, G->bt_bz, G->bt_qb, G->bt_group);
 }
 
 }  // namespace cbct

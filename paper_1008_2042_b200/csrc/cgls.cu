@@ -9,13 +9,19 @@
 
 namespace cbct {
 
+// float4 accesses only where every base pointer is 16-byte aligned (cbct.h asks for it; a misaligned vector access is
+// an SM exception, so the kernels check and fall back to scalar accesses instead of trusting the caller)
+__device__ __forceinline__ bool aligned16(const void *a, const void *b = nullptr) {
+    return ((reinterpret_cast<uintptr_t>(a) | reinterpret_cast<uintptr_t>(b)) & 15) == 0;
+}
+
 enum { S_GAMMA = 0, S_QQ = 1, S_ALPHA = 2, S_BETA = 3, S_RR = 4, S_GAMMA_NEW = 5, S_COUNT = 8 };
 
 // ||v||^2 -> *out.  Block partials in fp64, the last block to finish sums them in index order.
 __global__ void __launch_bounds__(256) sumsq_kernel(const float *__restrict__ v, long long n, double *out,
                                                     double *partials, unsigned int *counter) {
     double acc = 0.0;
-    const long long n4 = n >> 2;
+    const long long n4 = aligned16(v) ? n >> 2 : 0;
     const float4 *v4 = reinterpret_cast<const float4 *>(v);
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) {
         const float4 a = __ldg(v4 + i);
@@ -73,7 +79,7 @@ __global__ void cgls_beta_kernel(double *s, const int *flag) {
 __global__ void __launch_bounds__(256) axpy_dev_kernel(float *__restrict__ y, const float *__restrict__ x, long long n,
                                                        const double *s, float sign) {
     const float a = sign * (float)s[S_ALPHA];
-    const long long n4 = n >> 2;
+    const long long n4 = aligned16(y, x) ? n >> 2 : 0;
     float4 *y4 = reinterpret_cast<float4 *>(y);
     const float4 *x4 = reinterpret_cast<const float4 *>(x);
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) {
@@ -92,7 +98,7 @@ __global__ void __launch_bounds__(256) p_update_kernel(float *__restrict__ p, co
                                                        const double *s, const int *flag) {
     if (*flag) return;
     const float b = (float)s[S_BETA];
-    const long long n4 = n >> 2;
+    const long long n4 = aligned16(p, sv) ? n >> 2 : 0;
     float4 *p4 = reinterpret_cast<float4 *>(p);
     const float4 *s4 = reinterpret_cast<const float4 *>(sv);
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) {
@@ -163,6 +169,7 @@ extern "C" int cbct_cgls_init(cbct_cgls *cg, const float *d_g, const float *d_x,
     if (!cg || !d_g || !d_x || !d_r || !d_p) return CBCT_E_INVALID;
     cudaStream_t st = as_stream(stream);
     const cbct_geometry *G = cg->geom;
+    CBCT_TRY(device_error_pending(G));
     cgls_reset_kernel<<<1, 1, 0, st>>>(cg->d_scal, cg->d_flag);
     CBCT_LAUNCH_CHECK();
     CBCT_TRY(launch_forward(G, d_x, cg->d_q, st));                                   // q = P x0

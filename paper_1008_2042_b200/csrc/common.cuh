@@ -53,6 +53,13 @@ struct DevGeom {
     const double2 *view_cs;                      // device: (cos th, sin th) per view
 };
 
+// device error word of a geometry handle (see cbct_geometry_status in include/cbct.h): `dev` lives in device memory
+// (kernels OR their code into it and poll it at CTA start), `host` is the device alias of a mapped pinned host int that
+// the entry points read without synchronising.
+struct DevErr { int *dev; int *host; };
+enum { DEV_ERR_WAIT_TIMEOUT = CBCT_STATUS_WAIT_TIMEOUT, DEV_ERR_FW_RANGE = CBCT_STATUS_FORWARD_RANGE,
+       DEV_ERR_BT_RANGE = CBCT_STATUS_BACKPROJECT_RANGE };
+
 struct RayF {                                    // one ray in index space, fp32: P(tau) = c + b*tau
     float cx, cy, cz, bx, by, bz;
 };
@@ -115,6 +122,15 @@ struct cbct_geometry {
     float *d_bp_partial;                // P^T workspace: 8 per-corner partial volumes over the (n+1)^3 cells
     float *d_bp_projT;                  // P^T workspace: projections transposed to [view][iu][iv]
     cbct::BpTables bp;                  // P^T lookup tables (device pointers + constants)
+    // Which kernels run for this handle: decided ONCE, in cbct_geometry_create (plan + the CBCT_* selection variables read
+    // there, include/cbct.h), reported by cbct_geometry_describe; launches never re-route and never read the environment.
+    int fw_impl;                            // FW_TMA / FW_TILED / FW_GLOBAL
+    int fw_packed;                          // forward_tma_kernel: packed-pair (1) or scalar (0) instruction stream
+    int bp_impl;                            // BP_SCATTER / BP_CELL / BP_GATHER
+    int bt_packed;                          // backproject_scatter_kernel: packed-pair (1) or scalar (0) stream
+    // device error word (cbct_geometry_status): device int + mapped pinned host int
+    cbct::DevErr err;
+    int *h_err;                             // host address of the mapped word
     // forward TMA path (forward_tma.cu): box plan, y-fastest volume copy and its tensor map
     int fw_tma_ok, fw_b, fw_bs, fw_bz;      // box: fw_b columns (= row pitch) x fw_bs rows x fw_bz planes
     float fw_margin;
@@ -129,7 +145,7 @@ struct cbct_geometry {
     unsigned *d_bt_absmax;
     alignas(64) unsigned char bt_map_x[128];
     alignas(64) unsigned char bt_map_y[128];
-    // Siddon pair (siddon.cu), allocated at the first call: y-fastest volume copy, two int32 accumulator volumes, max|g|
+    // Siddon pair (siddon.cu), allocated by cbct_siddon_prepare: y-fastest volume copy, two int32 accumulator volumes, max|g|
     float *d_sd_volT;
     int *d_sd_acc;
     unsigned *d_sd_absmax;
@@ -146,7 +162,22 @@ struct cbct_cgls {
     unsigned int *d_counter;
 };
 
+// Default instruction stream / lane layout of the TMA kernels (overridden per handle by CBCT_FW_PACKED, CBCT_BT_PACKED,
+// CBCT_BT_LANES at cbct_geometry_create).
+#define CBCT_DEFAULT_FW_PACKED 0
+#define CBCT_DEFAULT_BT_PACKED 0
+#define CBCT_DEFAULT_BT_LANES 1
+
 namespace cbct {
+enum { FW_TMA = 0, FW_TILED = 1, FW_GLOBAL = 2 };
+enum { BP_SCATTER = 0, BP_CELL = 1, BP_GATHER = 2 };
+bool forward_tiled_fits(const cbct_geometry *G, float *margin_out);
+void describe_forward_tma(const cbct_geometry *G, char *buf, size_t cap);
+void describe_backproject_tma(const cbct_geometry *G, char *buf, size_t cap);
+// CBCT_E_DEVICE if a kernel of this handle has raised the device error word (read from the mapped host word: no sync)
+static inline int device_error_pending(const cbct_geometry *G) {
+    return (G->h_err && *reinterpret_cast<volatile int *>(G->h_err)) ? CBCT_E_DEVICE : CBCT_OK;
+}
 // kernels' host launchers used across translation units
 int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
 int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);

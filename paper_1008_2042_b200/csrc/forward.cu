@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(256) forward_tiled_kernel(DevGeom g, const flo
 }
 
 // can every single-sample slice of a 32x8 tile fit the shared-memory box?  (conservative, host side)
-static bool tiled_fits(const cbct_geometry *G, float *margin_out) {
+bool forward_tiled_fits(const cbct_geometry *G, float *margin_out) {
     const cbct_geometry_desc &d = G->desc;
     const double far = (d.sad + G->R) / d.sdd;                       // magnification bound inside the volume
     const double half_diag = 0.5 * std::sqrt((FW_TU * d.du) * (FW_TU * d.du) + (FW_TV * d.dv) * (FW_TV * d.dv));
@@ -236,14 +236,16 @@ int launch_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, cu
     const DevGeom &g = G->dg;
     ProfScope prof(PROF_FORWARD, st);
     dim3 block(FW_TU, FW_TV), grid(cdiv(g.nu, FW_TU), cdiv(g.nv, FW_TV), g.n_views);
+    CBCT_TRY(device_error_pending(G));
+    // the implementation was fixed at cbct_geometry_create (G->fw_impl): a failure here is returned, never re-routed
+    if (G->fw_impl == FW_TMA) return launch_forward_tma(G, d_vol, d_proj, st);
     float margin = 0.f;
-    const char *impl = getenv("CBCT_FORWARD_IMPL");                  // "global" / "tiled" force the older kernels (tests)
-    const bool want_global = impl && impl[0] == 'g', want_tiled = impl && impl[0] == 't' && impl[1] == 'i';
-    if (!want_global && !want_tiled && launch_forward_tma(G, d_vol, d_proj, st) == CBCT_OK) return CBCT_OK;
-    if (!want_global && tiled_fits(G, &margin))
+    if (G->fw_impl == FW_TILED) {
+        if (!forward_tiled_fits(G, &margin)) return CBCT_E_UNSUPPORTED;
         forward_tiled_kernel<<<grid, block, 0, st>>>(g, d_vol, d_proj, margin);
-    else
+    } else {
         forward_global_kernel<<<grid, block, 0, st>>>(g, d_vol, d_proj);
+    }
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

@@ -12,7 +12,7 @@
 //   * floor/fraction use the add-magic-number trick in round-down mode (no conversion instructions)
 //     and positions are kept relative to the box origin.
 #include <cmath>
-#include <cstdlib>
+#include <cstdio>
 #include <cstring>
 
 #include "tma_common.cuh"
@@ -33,15 +33,16 @@ template <int BF, int BS, bool PK>
 __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
                                                                  const float *__restrict__ vol, float *__restrict__ proj,
-                                                                 float margin, int bfs, int bss, int bzz, int dbg) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
+                                                                 float margin, int bfs, int bss, int bzz, DevErr err) {
+    extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2];
     __shared__ RayL corner[4];
     __shared__ ChunkPlan plans[2];
-    __shared__ int s_klo, s_khi;
-    float *buf0 = reinterpret_cast<float *>(smem_raw);
+    __shared__ int s_klo, s_khi, s_abort;
+    float *buf0 = reinterpret_cast<float *>(align128(smem_raw));   // the launch reserves 128 bytes for this
     const int box_elems = (bfs * bss * bzz + 31) & ~31;   // buffer stride: keeps the second buffer 128-byte aligned
     const unsigned box_bytes = (unsigned)(bfs * bss * bzz) * 4u;
+    const unsigned tx_bytes = box_bytes + (CBCT_FAULT(1) ? 16u : 0u);      // CBCT_FAULT: 0 outside the host-side test build
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // a warp covers 8(u) x 4(v) pixels: <= 10 columns of the fast axis, <= 2 rows, <= 2 z-planes
@@ -81,11 +82,13 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
 
     if (tid == 0) {
         s_klo = 0x7fffffff; s_khi = -1;
+        s_abort = *reinterpret_cast<volatile int *>(err.dev);      // an earlier CTA / call already failed: do nothing
         mbar_init(smem_u32(&bars[0]), 1); mbar_init(smem_u32(&bars[1]), 1);
         fence_mbar_init();
     }
     if ((tu == 0 || tu == FT_TU - 1) && (tv == 0 || tv == FT_TV - 1)) corner[(tv ? 2 : 0) + (tu ? 1 : 0)] = rl;
     __syncthreads();
+    if (s_abort) return;
     {
         const int wlo = __reduce_min_sync(0xffffffffu, klo), whi = __reduce_max_sync(0xffffffffu, khi);
         if (lane == 0) { atomicMin(&s_klo, wlo); atomicMax(&s_khi, whi); }
@@ -102,8 +105,8 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
         if (tid == 0) {
             const ChunkPlan p0 = plan_chunk(g, corner, K0, K1, margin, bfs, bss, bzz);
             plans[0] = p0;
-            if (p0.box.fits && !(dbg & 1)) {
-                mbar_expect_tx(smem_u32(&bars[0]), box_bytes);
+            if (p0.box.fits) {
+                mbar_expect_tx(smem_u32(&bars[0]), tx_bytes);
                 if (yfast) tma_load_3d(smem_u32(buf0), &map_y, p0.box.lf, p0.box.ls, p0.box.lz, smem_u32(&bars[0]));
                 else tma_load_3d(smem_u32(buf0), &map_x, p0.box.lf, p0.box.ls, p0.box.lz, smem_u32(&bars[0]));
             }
@@ -111,15 +114,18 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
         __syncthreads();
         unsigned phase0 = 0, phase1 = 0;
         int k0 = K0, stage = 0;
+        bool failed = false;
         while (k0 <= K1) {
             const ChunkPlan cur = plans[stage];
             const int kn = k0 + cur.kc;
+            bool next_in_flight = false;                 // thread 0: a copy into the other buffer has been issued
             if (tid == 0 && kn <= K1) {                  // the other buffer and plan slot were released by the barrier below
                 const ChunkPlan nx_ = plan_chunk(g, corner, kn, K1, margin, bfs, bss, bzz);
                 plans[stage ^ 1] = nx_;
-                if (nx_.box.fits && !(dbg & 1)) {
+                if (nx_.box.fits) {
+                    next_in_flight = true;
                     const unsigned bar = smem_u32(&bars[stage ^ 1]);
-                    mbar_expect_tx(bar, box_bytes);
+                    mbar_expect_tx(bar, tx_bytes);
                     const unsigned dst = smem_u32(buf0 + (stage ^ 1) * box_elems);
                     if (yfast) tma_load_3d(dst, &map_y, nx_.box.lf, nx_.box.ls, nx_.box.lz, bar);
                     else tma_load_3d(dst, &map_x, nx_.box.lf, nx_.box.ls, nx_.box.lz, bar);
@@ -127,9 +133,12 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
             }
             const int ja = max(k0, klo), jb = min(kn - 1, khi);
             if (cur.box.fits) {
-                if (!(dbg & 1)) mbar_wait(smem_u32(&bars[stage]), stage ? phase1 : phase0);
+                if (!mbar_wait_bounded(smem_u32(&bars[stage]), stage ? phase1 : phase0)) {
+                    failed = true;                        // the box never arrived: error status, no hang
+                    raise_device_error(err, DEV_ERR_WAIT_TIMEOUT);
+                }
                 if (stage) phase1 ^= 1; else phase0 ^= 1;
-                if (ja <= jb && !(dbg & 2)) {
+                if (ja <= jb && !failed) {
                     // local coordinates: sample j sits at F0 + (j - ja) * sF, etc.
                     const float tau_a = fmaf((float)(ja - k0), stepf, cur.tau_base);
                     const float F0 = fmaf(rl.bf, tau_a, rl.cf - (float)cur.box.lf);
@@ -141,7 +150,9 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                     const float pSf = (float)pS, pZf = (float)pZ;
                     float part = 0.f, jf = 0.f;
                     const int n = jb - ja + 1;
-                    if constexpr (PK && BF > 0) {
+                    if (!(run_inside(F0, sF, n, bfs) && run_inside(S0, sS, n, bss) && run_inside(Z0, sZ, n, bzz))) {
+                        raise_device_error(err, DEV_ERR_FW_RANGE);      // never index outside the box: skip, report
+                    } else if constexpr (PK && BF > 0) {
                         // Two samples (j, j+1) per iteration, one in each lane of a pair: positions, floors, fractions, the
                         // element index and all seven lerps are pair instructions.  The two contributions are added to `part`
                         // one after the other, so the sum is formed in the scalar stream's order.
@@ -249,7 +260,12 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                 }
                 total += part;
             }
-            __syncthreads();                              // everyone is done with buffer `stage`; next plan is visible
+            // everyone is done with buffer `stage`; next plan is visible; did anybody give up?
+            if (__syncthreads_or(failed ? 1 : 0)) {
+                // leave through the normal exit path, but not while a copy into this CTA's shared memory may still land
+                if (tid == 0 && next_in_flight) (void)mbar_wait_bounded(smem_u32(&bars[stage ^ 1]), (stage ^ 1) ? phase1 : phase0);
+                break;
+            }
             k0 = kn; stage ^= 1;
         }
     }
@@ -273,18 +289,16 @@ __global__ void __launch_bounds__(256) transpose_vol_kernel(const float *__restr
 }
 
 
-typedef void (*TmaKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, float *, float, int, int, int, int);
-// CBCT_FW_PACKED=0 selects the scalar instruction stream (same results); default: packed pairs
-static bool forward_packed() {
-    const char *e = getenv("CBCT_FW_PACKED");
-    return !(e && atoi(e) == 0);
-}
+typedef void (*TmaKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, float *, float, int, int, int, DevErr);
 static TmaKernel tma_kernel_ptr(int bf, int bs, bool pk) {
 #define CBCT_FK(F, S) if (bf == F && bs == S) return pk ? forward_tma_kernel<F, S, true> : forward_tma_kernel<F, S, false>;
     CBCT_FK(24, 22) CBCT_FK(40, 30) CBCT_FK(40, 38) CBCT_FK(56, 46) CBCT_FK(56, 54)
 #undef CBCT_FK
     return nullptr;
 }
+
+// two boxes (each a multiple of 128 bytes) + 128 bytes for the in-kernel alignment of the base
+static size_t fw_tma_smem_bytes(int bf, int bs, int bz) { return (size_t)2 * ((bf * bs * bz + 31) & ~31) * 4 + 128; }
 
 // choose the box for this geometry (once, at create); fw_tma_ok = 0 when the TMA path cannot be used
 void plan_forward_tma(cbct_geometry *G) {
@@ -322,7 +336,7 @@ void plan_forward_tma(cbct_geometry *G) {
     std::memcpy(G->fw_map_y, &m, sizeof(m));
     for (int pk = 0; pk < 2; ++pk) {
         const void *kern = reinterpret_cast<const void *>(tma_kernel_ptr(bf, bs, pk != 0));
-        if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) {
+        if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fw_tma_smem_bytes(bf, bs, bz)) != cudaSuccess) {
             (void)cudaGetLastError();
             return;
         }
@@ -331,7 +345,8 @@ void plan_forward_tma(cbct_geometry *G) {
 }
 
 int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st) {
-    if (!G->fw_tma_ok || (reinterpret_cast<uintptr_t>(d_vol) & 15)) return CBCT_E_UNSUPPORTED;
+    if (!G->fw_tma_ok) return CBCT_E_UNSUPPORTED;
+    if (reinterpret_cast<uintptr_t>(d_vol) & 15) return CBCT_E_INVALID;        // include/cbct.h: device pointers are 16-byte aligned
     const DevGeom &g = G->dg;
     CUtensorMap mx, my;
     if (!make_map(&mx, d_vol, g.nx, g.ny, g.nz, G->fw_b, G->fw_bs, G->fw_bz)) return CBCT_E_UNSUPPORTED;
@@ -341,14 +356,19 @@ int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj
         transpose_vol_kernel<<<grid, block, 0, st>>>(d_vol, G->d_fw_volT, g.nx, g.ny);
         CBCT_LAUNCH_CHECK();
     }
-    const size_t smem = (size_t)2 * ((G->fw_b * G->fw_bs * G->fw_bz + 31) & ~31) * 4;
+    const size_t smem = fw_tma_smem_bytes(G->fw_b, G->fw_bs, G->fw_bz);
     dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), g.n_views);
-    TmaKernel kern = tma_kernel_ptr(G->fw_b, G->fw_bs, forward_packed());
+    TmaKernel kern = tma_kernel_ptr(G->fw_b, G->fw_bs, G->fw_packed != 0);
     if (!kern) return CBCT_E_UNSUPPORTED;
-    kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz,
-                                                       getenv("CBCT_TMA_DEBUG") ? atoi(getenv("CBCT_TMA_DEBUG")) : 0);
+    kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz, G->err);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
+}
+
+// "forward_tma_kernel<40,30,packed> box 40x30x7" -- what cbct_geometry_describe reports for P
+void describe_forward_tma(const cbct_geometry *G, char *buf, size_t cap) {
+    snprintf(buf, cap, "forward_tma_kernel<%d,%d,%s> box %dx%dx%d", G->fw_b, G->fw_bs, G->fw_packed ? "packed" : "scalar", G->fw_b,
+             G->fw_bs, G->fw_bz);
 }
 
 }  // namespace cbct

@@ -2,11 +2,18 @@
 // cbct_geometry_create / _info: include/cbct.h; conventions of SURVEY.md §8(c) c.1-c.2.
 #include <atomic>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
 
+#include "../../include/cbct_debug.h"
 #include "common.cuh"
+
+#ifdef CBCT_TEST_FAULTS
+extern "C" int cbct_test_fault = 0;       // host-side test build only (tma_common.cuh)
+#endif
 
 namespace cbct {
 
@@ -94,6 +101,7 @@ extern "C" const char *cbct_status_string(int status) {
         case CBCT_E_INVALID: return "invalid argument";
         case CBCT_E_UNSUPPORTED: return "unsupported device (needs compute capability 10.x, sm_100a)";
         case CBCT_E_CUDA: return "CUDA runtime error (see cbct_last_cuda_error)";
+        case CBCT_E_DEVICE: return "a kernel raised the device error word (see cbct_geometry_status)";
         case CBCT_BREAKDOWN: return "CGLS breakdown (gamma == 0 or ||q||^2 == 0)";
         default: return "unknown status";
     }
@@ -126,6 +134,23 @@ extern "C" int cbct_profile_end(double ms[2], int count[2]) {
     }
     g_prof.clear();
     return status;
+}
+
+// The selection variables of include/cbct.h, read once per cbct_geometry_create.  -1 = not forced.
+// Defaults: the variants that have passed the device parity suite (tests/test_gpu_projectors.py).
+struct Options { int fw_impl, bp_impl, fw_packed, bt_packed, bt_lanes; };
+static Options read_options() {
+    Options o{-1, -1, CBCT_DEFAULT_FW_PACKED, CBCT_DEFAULT_BT_PACKED, CBCT_DEFAULT_BT_LANES};
+    if (const char *e = getenv("CBCT_FORWARD_IMPL")) {
+        if (!strcmp(e, "tma")) o.fw_impl = FW_TMA; else if (!strcmp(e, "tiled")) o.fw_impl = FW_TILED; else if (!strcmp(e, "global")) o.fw_impl = FW_GLOBAL;
+    }
+    if (const char *e = getenv("CBCT_BACKPROJECT_IMPL")) {
+        if (!strcmp(e, "scatter")) o.bp_impl = BP_SCATTER; else if (!strcmp(e, "cell")) o.bp_impl = BP_CELL; else if (!strcmp(e, "gather")) o.bp_impl = BP_GATHER;
+    }
+    if (const char *e = getenv("CBCT_FW_PACKED")) o.fw_packed = atoi(e) != 0;
+    if (const char *e = getenv("CBCT_BT_PACKED")) o.bt_packed = atoi(e) != 0;
+    if (const char *e = getenv("CBCT_BT_LANES")) o.bt_lanes = atoi(e) == 1 ? 1 : 0;
+    return o;
 }
 
 static int validate(const cbct_geometry_desc *d, double *R_out, double *step_out) {
@@ -165,6 +190,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
     G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr; G->d_fw_volT = nullptr; G->fw_tma_ok = 0;
+    G->err = DevErr{nullptr, nullptr}; G->h_err = nullptr;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
     G->d_sd_volT = nullptr; G->d_sd_acc = nullptr; G->d_sd_absmax = nullptr; G->sd_qb = 0; G->sd_group = 0;
     G->bp = BpTables{};
@@ -176,6 +202,11 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     if (e == cudaSuccess) e = cudaMemcpy(G->d_view_cs, cs.data(), sizeof(double2) * cs.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&G->d_ws_vol, sizeof(float) * G->n_vox);
     if (e == cudaSuccess) e = cudaMalloc(&G->d_ws_proj, sizeof(float) * G->n_rays);
+    // device error word: a device int the kernels OR into, and a mapped pinned host int the entry points poll
+    if (e == cudaSuccess) e = cudaMalloc(&G->err.dev, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(G->err.dev, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void **>(&G->h_err), sizeof(int), cudaHostAllocMapped);
+    if (e == cudaSuccess) { *G->h_err = 0; e = cudaHostGetDevicePointer(reinterpret_cast<void **>(&G->err.host), G->h_err, 0); }
     if (e != cudaSuccess) { cbct_geometry_destroy(G); return set_cuda_error(e); }
     G->workspace_bytes = sizeof(double2) * cs.size() + sizeof(float) * (G->n_vox + G->n_rays);
 
@@ -193,9 +224,27 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     g.tau0 = G->t_min + 0.5 * step - desc->sad;
     g.view_cs = G->d_view_cs;
 
+    // ---- which kernels serve this handle: plan + the selection variables, read HERE and nowhere else (cbct.h) ----
+    const Options opt = read_options();
+    G->fw_packed = opt.fw_packed; G->bt_packed = opt.bt_packed; G->bt_lm = opt.bt_lanes;
     plan_forward_tma(G);
     plan_backproject_tma(G);
     {
+        float margin = 0.f;
+        const bool tiled_ok = forward_tiled_fits(G, &margin);
+        int want = opt.fw_impl;
+        if (want < 0) want = G->fw_tma_ok ? FW_TMA : (tiled_ok ? FW_TILED : FW_GLOBAL);
+        if ((want == FW_TMA && !G->fw_tma_ok) || (want == FW_TILED && !tiled_ok)) { cbct_geometry_destroy(G); return CBCT_E_UNSUPPORTED; }
+        G->fw_impl = want;
+        want = opt.bp_impl;
+        if (want < 0) want = G->bt_ok ? BP_SCATTER : BP_CELL;
+        if (want == BP_SCATTER && !G->bt_ok) { cbct_geometry_destroy(G); return CBCT_E_UNSUPPORTED; }
+        if (want == BP_CELL && desc->nz + 1 > 512) {
+            if (opt.bp_impl == BP_CELL) { cbct_geometry_destroy(G); return CBCT_E_UNSUPPORTED; }
+            want = BP_GATHER;                             // volumes too tall for the cell kernel's z-lanes
+        }
+        G->bp_impl = want;
+        if (G->bp_impl != BP_SCATTER) free_backproject_tma(G);       // accumulators of a path that will not run
         const int st_bp = build_bp_tables(G);
         if (st_bp != CBCT_OK) { cbct_geometry_destroy(G); return st_bp; }
     }
@@ -243,8 +292,35 @@ extern "C" int cbct_siddon_fixed_point_plan(const cbct_geometry_desc *desc, int3
     return CBCT_OK;
 }
 
+extern "C" int cbct_geometry_describe(const cbct_geometry *G, char *buf, size_t cap) {
+    if (!G || !buf || !cap) return CBCT_E_INVALID;
+    char fw[160], bp[200];
+    if (G->fw_impl == FW_TMA) describe_forward_tma(G, fw, sizeof fw);
+    else snprintf(fw, sizeof fw, "%s", G->fw_impl == FW_TILED ? "forward_tiled_kernel" : "forward_global_kernel");
+    if (G->bp_impl == BP_SCATTER) describe_backproject_tma(G, bp, sizeof bp);
+    else snprintf(bp, sizeof bp, "%s", G->bp_impl == BP_CELL ? "backproject_cell_kernel + backproject_combine_kernel" : "backproject_gather_kernel");
+    snprintf(buf, cap, "forward: %s; backproject: %s", fw, bp);
+    return CBCT_OK;
+}
+
+extern "C" int cbct_geometry_status(cbct_geometry *G, void *stream, int *flags, int clear) {
+    if (!G) return CBCT_E_INVALID;
+    CBCT_CUDA_TRY(cudaStreamSynchronize(as_stream(stream)));
+    int bits = 0;
+    CBCT_CUDA_TRY(cudaMemcpy(&bits, G->err.dev, sizeof(int), cudaMemcpyDeviceToHost));
+    bits |= *reinterpret_cast<volatile int *>(G->h_err);
+    if (flags) *flags = bits;
+    if (clear && bits) {
+        CBCT_CUDA_TRY(cudaMemset(G->err.dev, 0, sizeof(int)));
+        *reinterpret_cast<volatile int *>(G->h_err) = 0;
+    }
+    return bits ? CBCT_E_DEVICE : CBCT_OK;
+}
+
 extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     if (!G) return CBCT_OK;
+    cudaFree(G->err.dev);
+    if (G->h_err) cudaFreeHost(G->h_err);
     cudaFree(G->d_view_cs);
     cudaFree(G->d_ws_vol);
     cudaFree(G->d_ws_proj);

@@ -6,8 +6,8 @@
 // Rates per SM are measured with clock64() inside the kernel (one CTA of 1024 threads per SM, the slowest warp counts),
 // so they do not depend on knowing the SM clock; bandwidths are measured with CUDA events on the launching stream.
 #include <algorithm>
-#include <cstdlib>
 
+#include "../../include/cbct_debug.h"
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -106,12 +106,12 @@ __global__ void __launch_bounds__(256) mb_l2_red_kernel(int *dst, long long n, i
 using namespace cbct;
 
 // out[0] = the rate, out[1] = seconds (event time of the measured launch), out[2] = work items of that launch
-extern "C" int cbct_microbench(int kind, double out[3], void *stream) {
+extern "C" int cbct_microbench(int kind, int iters_arg, double out[3], void *stream) {
     if (!out || kind < 0 || kind > 7) return CBCT_E_INVALID;
     CBCT_TRY(device_supported());
     cudaStream_t st = as_stream(stream);
-    // CBCT_MB_ITERS shortens the timed loops (host-side checks of the kernels; the default is what is reported)
-    const int n_sm = 148, iters = getenv("CBCT_MB_ITERS") ? std::max(1, atoi(getenv("CBCT_MB_ITERS"))) : 2000;
+    // a caller may shorten the timed loops (host-side checks of the kernels); the default is what is reported
+    const int n_sm = 148, iters = iters_arg > 0 ? iters_arg : 2000;
     const int reps_rd = iters >= 2000 ? 20 : 1, reps_red = iters >= 2000 ? 4 : 1;
     struct Scratch {                                                   // released on every return path
         long long *cycles = nullptr;

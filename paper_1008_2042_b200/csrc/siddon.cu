@@ -184,12 +184,12 @@ bool siddon_fixed_point_plan(const cbct_geometry_desc &d, double R, int *qb_out,
     return true;
 }
 
-static int siddon_workspace(cbct_geometry *G, bool need_acc) {
+static int siddon_workspace(cbct_geometry *G) {
     if (!G->d_sd_volT) {
         CBCT_CUDA_TRY(cudaMalloc(&G->d_sd_volT, sizeof(float) * G->n_vox));
         G->workspace_bytes += sizeof(float) * G->n_vox;
     }
-    if (need_acc && !G->d_sd_acc) {
+    if (!G->d_sd_acc) {
         int qb = 0, group = 0;
         double w = 0;
         if (!siddon_fixed_point_plan(G->desc, G->R, &qb, &group, &w)) return CBCT_E_UNSUPPORTED;
@@ -210,11 +210,16 @@ void free_siddon(cbct_geometry *G) {
 
 using namespace cbct;
 
-extern "C" int cbct_siddon_forward(cbct_geometry *G, const float *d_vol, float *d_proj, void *stream) {
-    if (!G || !d_vol || !d_proj) return CBCT_E_INVALID;
+// allocates the pair's workspace (the only Siddon entry point that does); idempotent
+extern "C" int cbct_siddon_prepare(cbct_geometry *G) {
+    if (!G) return CBCT_E_INVALID;
     if (G->n_vox > 0x7fffffffLL) return CBCT_E_UNSUPPORTED;           // 32-bit voxel indices in the traversal
     CBCT_TRY(device_supported());
-    CBCT_TRY(siddon_workspace(G, false));
+    return siddon_workspace(G);
+}
+
+extern "C" int cbct_siddon_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, void *stream) {
+    if (!G || !d_vol || !d_proj || !G->d_sd_volT) return CBCT_E_INVALID;   // cbct_siddon_prepare first
     const DevGeom &g = G->dg;
     cudaStream_t st = as_stream(stream);
     {
@@ -228,11 +233,8 @@ extern "C" int cbct_siddon_forward(cbct_geometry *G, const float *d_vol, float *
     return CBCT_OK;
 }
 
-extern "C" int cbct_siddon_backproject(cbct_geometry *G, const float *d_proj, float *d_vol, void *stream) {
-    if (!G || !d_vol || !d_proj) return CBCT_E_INVALID;
-    if (G->n_vox > 0x7fffffffLL) return CBCT_E_UNSUPPORTED;
-    CBCT_TRY(device_supported());
-    CBCT_TRY(siddon_workspace(G, true));
+extern "C" int cbct_siddon_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, void *stream) {
+    if (!G || !d_vol || !d_proj || !G->d_sd_acc) return CBCT_E_INVALID;     // cbct_siddon_prepare first
     const DevGeom &g = G->dg;
     cudaStream_t st = as_stream(stream);
     CBCT_CUDA_TRY(cudaMemsetAsync(G->d_sd_absmax, 0, sizeof(unsigned), st));

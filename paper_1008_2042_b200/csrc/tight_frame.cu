@@ -3,8 +3,7 @@
 // Boundary: edge-replicate extension in D, exact matrix transpose in D^T:
 // for the symmetric filters h0, h2 the transpose is the flipped filter with edge-replicate extension
 // of alpha, for the antisymmetric h1 it is the flipped filter with SIGN-FLIPPED replicate extension.
-#include <cstdlib>
-
+#include "../../include/cbct_debug.h"
 #include "common.cuh"
 
 namespace cbct {
@@ -306,15 +305,17 @@ extern "C" int tf_shrink(float *d_alpha, float mu, int nx, int ny, int nz, void 
 
 extern "C" int tf_reconstruct(const float *d_alpha, float *d_f, int nx, int ny, int nz, void *stream) {
     CBCT_TRY(tf_check(d_alpha, d_f, nx, ny, nz));
-    // default: the separable z-marching kernel; CBCT_TF_RECONSTRUCT_IMPL=direct selects the 27 x 27-tap kernel (cross-check)
-    const char *impl = getenv("CBCT_TF_RECONSTRUCT_IMPL");
-    if (!(impl && impl[0] == 'd')) {
-        dim3 grid(cdiv(nx, TR_X), cdiv(ny, TR_Y), cdiv(nz, TR_ZSEG));
-        tf_reconstruct_march_kernel<<<grid, TR_THREADS, 0, as_stream(stream)>>>(d_alpha, d_f, nx, ny, nz);
-    } else {
-        dim3 block(32, 4), grid(cdiv(nx, 32), cdiv(ny, 4), nz);
-        tf_reconstruct_kernel<<<grid, block, 0, as_stream(stream)>>>(d_alpha, d_f, nx, ny, nz);
-    }
+    dim3 grid(cdiv(nx, TR_X), cdiv(ny, TR_Y), cdiv(nz, TR_ZSEG));
+    tf_reconstruct_march_kernel<<<grid, TR_THREADS, 0, as_stream(stream)>>>(d_alpha, d_f, nx, ny, nz);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+// cbct_debug.h: the 27 x 27-tap cross-check of the kernel above
+extern "C" int tf_reconstruct_direct(const float *d_alpha, float *d_f, int nx, int ny, int nz, void *stream) {
+    CBCT_TRY(tf_check(d_alpha, d_f, nx, ny, nz));
+    dim3 block(32, 4), grid(cdiv(nx, 32), cdiv(ny, 4), nz);
+    tf_reconstruct_kernel<<<grid, block, 0, as_stream(stream)>>>(d_alpha, d_f, nx, ny, nz);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

@@ -16,6 +16,54 @@ constexpr unsigned FT_MAGIC_BITS = 0x4B000000u;
 
 struct RayL { float cf, cs, cz, bf, bs, bz; };  // ray in (fast, slow, z) index coordinates: P(tau) = c + b tau
 
+// ---- "cannot hang, cannot fault" guards of the two TMA kernels ------------------------------------------------------------
+// (1) Every wait on an mbarrier is bounded by %globaltimer: on expiry the CTA raises DEV_ERR_WAIT_TIMEOUT and leaves
+//     through the normal exit path (a wrong transaction count or a lost copy becomes an error status, not a hung SM).
+// (2) Before a thread touches the shared-memory box of a chunk it checks that its FIRST and LAST sample of the chunk lie
+//     inside the box (positions are fma(j, s, P0): monotone in j, so the two ends bound every sample between them); a
+//     thread whose samples would leave the box raises DEV_ERR_*_RANGE and skips the chunk, so a planning mistake can
+//     never become an out-of-range shared-memory access.
+// (3) The dynamic shared-memory base is rounded up to 128 bytes in the kernel (TMA boxes need it), not assumed.
+constexpr unsigned long long CBCT_WAIT_NS = 200ull * 1000ull * 1000ull;      // 0.2 s: a box copy takes microseconds
+
+// Deliberate protocol mistakes, compiled ONLY into the host-side test build (tests/cpu_shim defines CBCT_TEST_FAULTS;
+// the product build never does, CBCT_FAULT(..) is the constant 0 there): they prove that the guards above turn a wrong
+// transaction count / a mis-planned box into an error status instead of a hang / an out-of-range access.
+#ifdef CBCT_TEST_FAULTS
+extern "C" int cbct_test_fault;      // 1: expect_tx announces 16 bytes too many; 2: forward box origin shifted; 4: scatter box origin shifted
+#define CBCT_FAULT(bit) (cbct_test_fault & (bit))
+#else
+#define CBCT_FAULT(bit) 0
+#endif
+
+__device__ __forceinline__ void raise_device_error(const DevErr &e, int code) {
+    atomicOr(e.dev, code);
+    *reinterpret_cast<volatile int *>(e.host) = code;      // mapped pinned host word: the next entry point sees it without a sync
+    __threadfence_system();
+}
+
+__device__ __forceinline__ bool mbar_wait_bounded(unsigned bar, unsigned parity) {
+    if (mbar_try_wait(bar, parity)) return true;
+    const unsigned long long t0 = globaltimer_ns();
+    for (;;) {
+#pragma unroll 1
+        for (int i = 0; i < 16; ++i)
+            if (mbar_try_wait(bar, parity)) return true;
+        if (globaltimer_ns() - t0 > CBCT_WAIT_NS) return false;
+    }
+}
+
+__device__ __forceinline__ unsigned char *align128(unsigned char *p) {
+    return p + ((128u - (smem_u32(p) & 127u)) & 127u);
+}
+
+// samples j = 0..n-1 at P0 + j*s: do all floors lie in [0, ext-2] (so that floor and floor+1 are inside the box)?
+__device__ __forceinline__ bool run_inside(float P0, float s, int n, int ext) {
+    const float Pe = fmaf((float)(n - 1), s, P0);
+    const float lo = fminf(P0, Pe), hi = fmaxf(P0, Pe);
+    return lo >= 0.f && hi < (float)(ext - 1);
+}
+
 struct Box3 { int lf, ls, lz; bool fits; };
 
 // origin of the box for samples tau_a..tau_b of the tile (AABB of the 4 corner rays at both ends grown by
@@ -56,6 +104,7 @@ __device__ __forceinline__ ChunkPlan plan_chunk(const DevGeom &g, const RayL *co
         kc = (kc > 8) ? (kc * 3) >> 2 : kc - 1;            // 64, 48, 36, 27, 20, 15, 11, 8, 7, ...
     }
     p.kc = kc;
+    if (CBCT_FAULT(2 | 4)) p.box.ls += 5;                  // test build only: a box that does not cover its samples
     return p;
 }
 

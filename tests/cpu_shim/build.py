@@ -20,7 +20,7 @@ import cu2cpp  # noqa: E402
 # -mfma + contraction: a*b+c becomes one fused multiply-add, as nvcc's default -fmad=true does on the device
 # SHIM_CXX_EXTRA="-fsanitize=alignment,bounds -fno-sanitize-recover=all" adds UBSan's checks of vector-typed accesses and fixed arrays
 EXTRA = os.environ.get("SHIM_CXX_EXTRA", "").split()
-CXXFLAGS = EXTRA + ["-std=c++17", "-O2", "-g", "-fPIC", "-fopenmp", "-mavx2", "-mfma", "-ffp-contract=fast", "-fno-strict-aliasing",
+CXXFLAGS = EXTRA + ["-DCBCT_TEST_FAULTS", "-std=c++17", "-O2", "-g", "-fPIC", "-fopenmp", "-mavx2", "-mfma", "-ffp-contract=fast", "-fno-strict-aliasing",
             "-Wno-unknown-pragmas", "-Wno-attributes",
             "-I", os.path.join(HERE, "include"), "-I", CSRC, "-I", os.path.join(ROOT, "include"), "-include", "shim_ptx.h"]
 

@@ -66,6 +66,10 @@ static inline cudaError_t cudaMalloc(T **p, size_t bytes) {
     return *p ? cudaSuccess : cudaErrorMemoryAllocation;
 }
 static inline cudaError_t cudaFree(void *p) { shim::dev_free(p); return cudaSuccess; }
+enum { cudaHostAllocMapped = 2 };
+static inline cudaError_t cudaHostAlloc(void **p, size_t bytes, unsigned) { *p = shim::dev_malloc(bytes); return *p ? cudaSuccess : cudaErrorMemoryAllocation; }
+static inline cudaError_t cudaHostGetDevicePointer(void **dp, void *hp, unsigned) { *dp = hp; return cudaSuccess; }   // one address space
+static inline cudaError_t cudaFreeHost(void *p) { shim::dev_free(p); return cudaSuccess; }
 static inline cudaError_t cudaGetLastError() { return cudaSuccess; }
 static inline cudaError_t cudaMemcpy(void *d, const void *s, size_t n, cudaMemcpyKind) { std::memcpy(d, s, n); return cudaSuccess; }
 static inline cudaError_t cudaMemcpyAsync(void *d, const void *s, size_t n, cudaMemcpyKind, cudaStream_t = nullptr) {
@@ -109,6 +113,9 @@ uint64_t warp_collective(unsigned mask, WarpOp op, uint64_t payload, int arg);
 }
 #define SHIM_LAUNCH(...) ::shim::launch_kernel(__VA_ARGS__)
 static inline void __syncthreads() { shim::syncthreads(); }
+namespace shim { int syncthreads_or(int pred); }
+static inline int __syncthreads_or(int pred) { return shim::syncthreads_or(pred); }
+static inline void __threadfence_system() { __atomic_thread_fence(__ATOMIC_SEQ_CST); }
 static inline void __syncwarp(unsigned mask = 0xffffffffu) { shim::warp_collective(mask, shim::W_BALLOT, 0, 0); }
 static inline long long clock64() { return (long long)__builtin_ia32_rdtsc(); }
 static inline void __threadfence() { __atomic_thread_fence(__ATOMIC_SEQ_CST); }
@@ -147,6 +154,7 @@ static inline T shim_atomic_minmax(T *p, T v, bool is_max) {
     while ((is_max ? v > old : v < old) && !__atomic_compare_exchange_n(p, &old, v, true, __ATOMIC_RELAXED, __ATOMIC_RELAXED)) {}
     return old;
 }
+static inline int atomicOr(int *p, int v) { return __atomic_fetch_or(p, v, __ATOMIC_RELAXED); }
 static inline int atomicMax(int *p, int v) { return shim_atomic_minmax(p, v, true); }
 static inline unsigned atomicMax(unsigned *p, unsigned v) { return shim_atomic_minmax(p, v, true); }
 static inline int atomicMin(int *p, int v) { return shim_atomic_minmax(p, v, false); }

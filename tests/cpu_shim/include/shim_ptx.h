@@ -15,7 +15,8 @@
 namespace shim {
 void mbar_init(unsigned bar, unsigned count);
 void mbar_expect_tx(unsigned bar, unsigned bytes);
-void mbar_wait(unsigned bar, unsigned parity);
+bool mbar_try_wait(unsigned bar, unsigned parity);   // one poll: lets the other fibers run, true once the phase completed
+unsigned long long globaltimer_ns();                 // virtual clock of the block: jumps ahead when every live fiber only polls
 void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar);
 void tma_reduce_add_3d(const CUtensorMap *map, int c0, int c1, int c2, unsigned src);
 void bulk_commit();
@@ -29,7 +30,8 @@ static inline unsigned smem_u32(const void *p) { return shim::cvta_shared(p); }
 static inline void mbar_init(unsigned bar, unsigned count) { shim::mbar_init(bar, count); }
 static inline void fence_mbar_init() {}
 static inline void mbar_expect_tx(unsigned bar, unsigned bytes) { shim::mbar_expect_tx(bar, bytes); }
-static inline void mbar_wait(unsigned bar, unsigned parity) { shim::mbar_wait(bar, parity); }
+static inline bool mbar_try_wait(unsigned bar, unsigned parity) { return shim::mbar_try_wait(bar, parity); }
+static inline unsigned long long globaltimer_ns() { return shim::globaltimer_ns(); }
 static inline void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar) {
     shim::tma_load_3d(dst, map, c0, c1, c2, bar);
 }

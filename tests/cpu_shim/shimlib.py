@@ -147,10 +147,23 @@ class Geometry:
         return self._call("cbct_backproject_eq3", g, self.vol_shape)
 
     def siddon_forward(self, f):
+        check(lib().cbct_siddon_prepare(self.handle), "cbct_siddon_prepare")
         return self._call("cbct_siddon_forward", f, self.proj_shape)
 
     def siddon_backproject(self, g):
+        check(lib().cbct_siddon_prepare(self.handle), "cbct_siddon_prepare")
         return self._call("cbct_siddon_backproject", g, self.vol_shape)
+
+    def describe(self):
+        buf = C.create_string_buffer(512)
+        check(lib().cbct_geometry_describe(self.handle, buf, len(buf)), "cbct_geometry_describe")
+        return buf.value.decode()
+
+    def status(self, clear=False):
+        """(status code, flags) of cbct_geometry_status"""
+        flags = C.c_int(0)
+        s = lib().cbct_geometry_status(self.handle, None, C.byref(flags), int(clear))
+        return s, flags.value
 
 
 class Cgls:
@@ -193,9 +206,10 @@ def tf_shrink(alpha, mu):
     return alpha
 
 
-def tf_reconstruct(alpha):
+def tf_reconstruct(alpha, direct=False):
     out = Buf(alpha.shape[1:])
-    check(lib().tf_reconstruct(alpha.ptr, out.ptr, *_dims(out.shape), None), "tf_reconstruct")
+    fn = lib().tf_reconstruct_direct if direct else lib().tf_reconstruct
+    check(fn(alpha.ptr, out.ptr, *_dims(out.shape), None), "tf_reconstruct")
     return out
 
 

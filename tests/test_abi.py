@@ -15,9 +15,11 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "cbct.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    names = re.findall(r"\b(?:int|long long|const char \*)\s*\*?\s*((?:cbct|tf|mg)_\w+)\s*\(", text)
+    names = []
+    for header in ("cbct.h", "cbct_debug.h"):        # the product ABI and the probes
+        text = open(os.path.join(ROOT, "include", header)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names += re.findall(r"\b(?:int|long long|const char \*)\s*\*?\s*((?:cbct|tf|mg)_\w+)\s*\(", text)
     return sorted(set(names))
 
 
@@ -38,7 +40,7 @@ def test_header_symbols_are_exported(cdll):
 def test_status_strings_and_version(cdll):
     cdll.cbct_status_string.restype = ctypes.c_char_p
     assert cdll.cbct_status_string(0) == b"ok"
-    for code in (-1, -2, -3, 1):
+    for code in (-1, -2, -3, -4, 1):
         assert len(cdll.cbct_status_string(code)) > 3
     assert cdll.cbct_version() >= 100
     assert cdll.cbct_last_cuda_error() == 0

@@ -78,12 +78,11 @@ def test_tf_three_call_path(shape):
 
 @pytest.mark.parametrize("impl", ["march", "direct"])
 @pytest.mark.parametrize("shape", SHAPES + [(31, 20, 45)])
-def test_tf_reconstruct_both_kernels(monkeypatch, shape, impl):
+def test_tf_reconstruct_both_kernels(shape, impl):
     rng = np.random.default_rng(sum(shape) + 1)
     a = rng.standard_normal((27,) + shape).astype(np.float32)
-    monkeypatch.setenv("CBCT_TF_RECONSTRUCT_IMPL", impl)
     sl.kernel_log()
-    out = sl.tf_reconstruct(sl.dev(a)).numpy()
+    out = sl.tf_reconstruct(sl.dev(a), direct=(impl == "direct")).numpy()
     assert sl.kernel_log() == ["cbct::tf_reconstruct_march_kernel" if impl == "march" else "cbct::tf_reconstruct_kernel"]
     r_ref = osv.tf_reconstruct(a.astype(np.float64))
     assert np.max(np.abs(out - r_ref)) <= 1e-5 * np.max(np.abs(r_ref))
@@ -128,13 +127,12 @@ def test_multigrid_a2_driver_two_levels():
     assert rel(out, ref) <= 1e-4
 
 
-def test_microbench_kernels_stay_in_bounds(monkeypatch):
+def test_microbench_kernels_stay_in_bounds():
     """cbct_microbench (SURVEY.md §8(d) denominators) with its timed loops shortened: every kernel runs under the shim's
     guards and alignment checks; the rates themselves mean nothing on the host."""
     import ctypes as C
-    monkeypatch.setenv("CBCT_MB_ITERS", "1")
     for kind in range(8):
         out = (C.c_double * 3)()
-        sl.check(sl.lib().cbct_microbench(kind, out, None), f"cbct_microbench({kind})")
+        sl.check(sl.lib().cbct_microbench(kind, 1, out, None), f"cbct_microbench({kind})")
         assert out[2] > 0
-    assert sl.lib().cbct_microbench(8, out, None) == -1
+    assert sl.lib().cbct_microbench(8, 1, out, None) == -1

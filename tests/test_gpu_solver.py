@@ -154,15 +154,14 @@ def test_tf_three_call_path(shape):
 
 @pytest.mark.parametrize("impl", ["march", "direct"])
 @pytest.mark.parametrize("shape", SHAPES + [(31, 20, 45)])
-def test_tf_reconstruct_both_kernels(monkeypatch, shape, impl):
-    """D^T has two kernels: the separable z-marching one (default) and the direct 27x27-tap one
-    (CBCT_TF_RECONSTRUCT_IMPL=direct); several z-segments, ragged tiles, 1-thick axes."""
+def test_tf_reconstruct_both_kernels(shape, impl):
+    """D^T has two kernels: the separable z-marching one (tf_reconstruct) and the direct 27x27-tap one
+    (tf_reconstruct_direct, cbct_debug.h); several z-segments, ragged tiles, 1-thick axes."""
     rng = np.random.default_rng(sum(shape) + 1)
     a = rng.standard_normal((27,) + shape).astype(np.float32)
     d_a = dev(a)
     d_out = torch.empty(shape, dtype=torch.float32, device="cuda")
-    monkeypatch.setenv("CBCT_TF_RECONSTRUCT_IMPL", impl)
-    cb.tf_reconstruct(d_a, d_out)
+    (cb.tf_reconstruct_direct if impl == "direct" else cb.tf_reconstruct)(d_a, d_out)
     torch.cuda.synchronize()
     r_ref = osv.tf_reconstruct(a.astype(np.float64))
     assert np.max(np.abs(host(d_out) - r_ref)) <= 1e-5 * np.max(np.abs(r_ref))
