@@ -55,7 +55,9 @@ enum {
 enum {
     CBCT_STATUS_WAIT_TIMEOUT = 1,       /* a bounded mbarrier wait expired (TMA copy never completed) */
     CBCT_STATUS_FORWARD_RANGE = 2,      /* cbct_forward: a thread's samples left the staged box (skipped, not read) */
-    CBCT_STATUS_BACKPROJECT_RANGE = 4   /* cbct_backproject: a thread's samples left the accumulator box (skipped) */
+    CBCT_STATUS_BACKPROJECT_RANGE = 4,  /* cbct_backproject: a thread's samples left the accumulator box (skipped) */
+    CBCT_STATUS_FIXED_POINT_RANGE = 8   /* cbct_backproject: an int32 accumulator reached 2^30, half its range: the head-room
+                                           plan (cbct_backproject_fixed_point_plan) does not hold for this geometry / input */
 };
 
 /* Static string for a status code. */
@@ -153,10 +155,14 @@ int cbct_siddon_backproject(const cbct_geometry *geom, const float *d_proj, floa
 int cbct_siddon_fixed_point_plan(const cbct_geometry_desc *desc, int32_t *qb, int32_t *views_per_group, double *max_path_sum_per_view);
 
 /* Host arithmetic only (no device needed): the fixed-point plan cbct_backproject uses for this geometry.
- *   max_weight_sum_per_view: upper bound on the sum of trilinear weights one voxel receives from one view;
+ *   max_weight_sum_per_view: planned bound on the sum of trilinear weights one voxel receives from one view
+ *                    (1.25 x the largest continuum sample density x the under-sampling excess per axis; pinned
+ *                    against the oracle's exact sums in tests/test_abi.py);
  *   qb: contributions are rounded to multiples of max|g| / 2^qb;
- *   views_per_group: views accumulated in int32 before conversion to fp32
- *                    (views_per_group * max_weight_sum_per_view * 2^qb < 2^31, so the sums cannot wrap).
+ *   views_per_group: views accumulated in int32 before conversion to fp32:
+ *                    views_per_group * max_weight_sum_per_view * 2^qb <= 2^30, HALF the int32 range.  The conversion
+ *                    pass raises CBCT_STATUS_FIXED_POINT_RANGE if any accumulator reaches 2^30, so a geometry that
+ *                    exceeds the planned bound by up to 3x is reported (cbct_geometry_status), never wrapped silently.
  * Any out pointer may be NULL.  CBCT_E_INVALID as cbct_geometry_create; CBCT_E_UNSUPPORTED if no plan exists. */
 int cbct_backproject_fixed_point_plan(const cbct_geometry_desc *desc, int32_t *qb, int32_t *views_per_group,
                                       double *max_weight_sum_per_view);

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcbct_b200.so")
 
 CBCT_OK, CBCT_E_INVALID, CBCT_E_UNSUPPORTED, CBCT_E_CUDA, CBCT_E_DEVICE, CBCT_BREAKDOWN = 0, -1, -2, -3, -4, 1
-STATUS_BITS = {1: "wait_timeout", 2: "forward_range", 4: "backproject_range"}
+STATUS_BITS = {1: "wait_timeout", 2: "forward_range", 4: "backproject_range", 8: "fixed_point_range"}
 
 # every symbol include/cbct.h and include/cbct_debug.h declare (tests check the library exports all of them)
 EXPORTS = [

@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
     if constexpr (LM == 0) { tu = (warp & 1) * 8 + (lane & 7); tv = (warp >> 1) * 4 + (lane >> 3); }
     else { tu = lane & 15; tv = warp + 8 * (lane >> 4); }
     const int skew = LM == 0 ? 2 * (lane >> 3) : 0;
-    const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = view0 + blockIdx.z;
+    const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = g.view_order[view0 + blockIdx.z];
     const bool valid = iu < g.nu && iv < g.nv;
 
     const double2 cs = g.view_cs[view];
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
 __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y,
                                                                    float *__restrict__ vol, int nx, int ny, int pf, int ps, int pz,
                                                                    const unsigned *__restrict__ absmax_bits, float step_over_two_qb,
-                                                                   int accumulate) {
+                                                                   int accumulate, long long sat_limit, DevErr err) {
     __shared__ int tile[32][33];
     const size_t base = (size_t)blockIdx.z * nx * ny;
     const size_t base_x = ((size_t)(blockIdx.z + pz) * (ny + ps) + ps) * (nx + pf) + pf;     // acc_x[z+pz][ps][pf]
@@ -319,7 +319,15 @@ __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__
         const int x = x0 + threadIdx.x, y = y0 + j;
         if (x < nx && y < ny) {
             const size_t o = base + (size_t)y * nx + x;
-            const float v = (float)(__ldg(acc_x + base_x + (size_t)y * (nx + pf) + x) + tile[threadIdx.x][j]) * k;
+            const int ax = __ldg(acc_x + base_x + (size_t)y * (nx + pf) + x), ay = tile[threadIdx.x][j];
+            // head-room check: a sum that reached sat_limit (half the int32 range for cbct_backproject) means the planned
+            // bound on the weight sums does not hold here; report it (a true sum below 3 x sat_limit cannot hide by wrapping)
+            const long long wide = (long long)ax + (long long)ay;
+            if (wide >= sat_limit || wide <= -sat_limit) {
+                atomicOr(err.dev, DEV_ERR_FIXED_POINT);
+                *reinterpret_cast<volatile int *>(err.host) = DEV_ERR_FIXED_POINT;
+            }
+            const float v = (float)wide * k;
             vol[o] = accumulate ? vol[o] + v : v;
         }
     }
@@ -339,19 +347,29 @@ static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm, bool pk) {
 }
 
 // Fixed-point plan of the scatter kernel (host arithmetic only; exported as cbct_backproject_fixed_point_plan).
-// w_view bounds the sum of trilinear weights one voxel can receive from ONE view: the continuum density of
-// samples (rays per area at the nearest depth, / step) times the voxel volume, times the worst-case excess of a
-// sum of hat samples over its mean when a sampling pitch exceeds the voxel pitch, times 1.5.  Then
-// views_per_group * w_view * 2^qb < 2^31 with qb <= 22 (the range of the rounding trick).
+// w_view is the planned bound on the sum of trilinear weights one voxel can receive from ONE view:
+//   * the largest continuum density of sample points, in samples per voxel volume.  The samples are the image of the
+//     lattice (iu, iv, k) under  x_S + t (d(u,v) - x_S) / L(u,v),  whose cell has the volume  du dv step t^2 SDD / L^3
+//     (t^2 / L^2 from the fan, SDD / L from the incidence on the flat panel): densest at the nearest depth t_min = SAD - R
+//     and for the most oblique ray, L_max;  the sum of the hat weights of a voxel is its integral (one voxel volume) times
+//     that density, when the lattice is fine against the voxel (measured with the oracle: 0.91 .. 0.98 of this figure at
+//     the five configs, tests/test_abi.py);
+//   * times, per lattice direction whose pitch exceeds the voxel pitch, that pitch ratio (one sample can sit on the peak
+//     of the hat while the mean spreads it over the pitch);
+//   * times 1.25.
+// Then views_per_group * w_view * 2^qb <= 2^30 with qb <= 22 (the range of the rounding trick): the plan uses HALF the
+// int32 range and backproject_finalize_kernel reports any accumulator that reaches 2^30, so a geometry that breaks the
+// bound by up to 3x is caught (CBCT_STATUS_FIXED_POINT_RANGE) instead of wrapping silently.
 bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int *qb_out, int *group_out, double *w_view_out) {
-    const double t_min = d.sad - R;
-    const double near = d.sdd / t_min, far = (d.sad + R) / d.sdd;
-    const double mean_w = d.dx * d.dy * d.dz * near * near / (d.du * d.dv * step);
+    const double t_min = d.sad - R, far = (d.sad + R) / d.sdd;
+    const double umax = std::fabs(d.u0) + 0.5 * d.nu * d.du, vmax = std::fabs(d.v0) + 0.5 * d.nv * d.dv;
+    const double l_max = std::sqrt(d.sdd * d.sdd + umax * umax + vmax * vmax);
+    const double mean_w = d.dx * d.dy * d.dz * l_max * l_max * l_max / (d.sdd * t_min * t_min * d.du * d.dv * step);
     const double su = std::fmax(1.0, d.du * far / std::fmin(d.dx, d.dy)), sv = std::fmax(1.0, d.dv * far / d.dz);
     const double st = std::fmax(1.0, step / std::fmin(d.dx, std::fmin(d.dy, d.dz)));
-    const double w_view = 1.5 * mean_w * su * sv * st;
+    const double w_view = 1.25 * mean_w * su * sv * st;
     int qb = 21, group = d.n_views;
-    const auto cap = [&](int bits) { return std::ldexp(1.0, 31 - bits) / w_view; };
+    const auto cap = [&](int bits) { return std::ldexp(1.0, 30 - bits) / w_view; };
     if (cap(22) >= d.n_views) qb = 22;
     else if (cap(21) >= d.n_views) qb = 21;
     else {
@@ -428,9 +446,11 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
     absmax_kernel<<<592, 256, 0, st>>>(d_proj, (long long)G->n_rays, G->d_bt_absmax);
     CBCT_LAUNCH_CHECK();
     const size_t smem = bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz);
-    const float two_qb = (float)std::ldexp(1.0, G->bt_qb);
-    for (int v0 = 0; v0 < g.n_views; v0 += G->bt_group) {
-        const int nv_ = std::min(G->bt_group, g.n_views - v0);
+    // CBCT_FAULT: 0 outside the host-side test build; there, 8 = ignore the head-room plan (all views in one group)
+    const int qb = G->bt_qb, group = CBCT_FAULT(8) ? g.n_views : G->bt_group;
+    const float two_qb = (float)std::ldexp(1.0, qb);
+    for (int v0 = 0; v0 < g.n_views; v0 += group) {          // view0 / blockIdx.z are positions in g.view_order
+        const int nv_ = std::min(group, g.n_views - v0);
         CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_acc, 0, sizeof(int) * G->bt_acc_elems, st));
         dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), nv_);
         kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_proj, G->d_bt_acc, G->d_bt_absmax, two_qb, v0, G->fw_margin, G->bt_bz, G->err);
@@ -438,7 +458,7 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
         dim3 fb(32, 8), fg(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
         backproject_finalize_kernel<<<fg, fb, 0, st>>>(G->d_bt_acc, G->d_bt_acc + G->bt_acc_y_off, d_vol, g.nx, g.ny, G->bt_b, G->bt_bs,
                                                        G->bt_bz, G->d_bt_absmax,
-                                                       (float)(G->step / std::ldexp(1.0, G->bt_qb)), v0 > 0 ? 1 : 0);
+                                                       (float)(G->step / std::ldexp(1.0, qb)), v0 > 0 ? 1 : 0, 1LL << 30, G->err);
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;

@@ -51,6 +51,11 @@ struct DevGeom {
     double inv_dx, inv_dy, inv_dz, cx, cy, cz;
     double tau0, step;
     const double2 *view_cs;                      // device: (cos th, sin th) per view
+    // device: a permutation of the views, those whose fast shared-memory axis is x first, then the y-fast ones (stable).
+    // The TMA kernels take their view from it (blockIdx.z is a POSITION in this order), so that each of the two
+    // orientation-specific copies of the volume / accumulator volumes is used in one contiguous phase of the launch and
+    // stays L2-resident during it (two 73 / 113 MB copies do not fit the 126 MB L2 together, one does).
+    const int *view_order;
 };
 
 // device error word of a geometry handle (see cbct_geometry_status in include/cbct.h): `dev` lives in device memory
@@ -58,7 +63,7 @@ struct DevGeom {
 // the entry points read without synchronising.
 struct DevErr { int *dev; int *host; };
 enum { DEV_ERR_WAIT_TIMEOUT = CBCT_STATUS_WAIT_TIMEOUT, DEV_ERR_FW_RANGE = CBCT_STATUS_FORWARD_RANGE,
-       DEV_ERR_BT_RANGE = CBCT_STATUS_BACKPROJECT_RANGE };
+       DEV_ERR_BT_RANGE = CBCT_STATUS_BACKPROJECT_RANGE, DEV_ERR_FIXED_POINT = CBCT_STATUS_FIXED_POINT_RANGE };
 
 struct RayF {                                    // one ray in index space, fp32: P(tau) = c + b*tau
     float cx, cy, cz, bx, by, bz;
@@ -118,6 +123,7 @@ struct cbct_geometry {
     int64_t n_vox, n_rays, n_samples;
     cbct::DevGeom dg;
     double2 *d_view_cs;
+    int *d_view_order;
     float *d_ws_vol, *d_ws_proj;        // staging for the *_host entry points (allocated at create)
     float *d_bp_partial;                // P^T workspace: 8 per-corner partial volumes over the (n+1)^3 cells
     float *d_bp_projT;                  // P^T workspace: projections transposed to [view][iu][iv]
@@ -162,12 +168,6 @@ struct cbct_cgls {
     unsigned int *d_counter;
 };
 
-// Default instruction stream / lane layout of the TMA kernels (overridden per handle by CBCT_FW_PACKED, CBCT_BT_PACKED,
-// CBCT_BT_LANES at cbct_geometry_create).
-#define CBCT_DEFAULT_FW_PACKED 0
-#define CBCT_DEFAULT_BT_PACKED 0
-#define CBCT_DEFAULT_BT_LANES 1
-
 namespace cbct {
 enum { FW_TMA = 0, FW_TILED = 1, FW_GLOBAL = 2 };
 enum { BP_SCATTER = 0, BP_CELL = 1, BP_GATHER = 2 };
@@ -194,7 +194,7 @@ __global__ void transpose_vol_kernel(const float *__restrict__ v, float *__restr
 __global__ void absmax_kernel(const float *__restrict__ g, long long n, unsigned *out);                        // backproject_tma.cu
 __global__ void backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y, float *__restrict__ vol,
                                             int nx, int ny, int pf, int ps, int pz, const unsigned *__restrict__ absmax_bits,
-                                            float step_over_two_qb, int accumulate);                             // backproject_tma.cu
+                                            float step_over_two_qb, int accumulate, long long sat_limit, DevErr err);  // backproject_tma.cu
 int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
 void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,

@@ -30,7 +30,7 @@ __device__ __forceinline__ float fetch0g(const float *__restrict__ vol, const De
 // positions, floors, fractions, element index and the seven lerps are all pair instructions.  Every lane is the same IEEE
 // operation in the same order as the scalar path, so both variants return bit-identical projections.
 template <int BF, int BS, bool PK>
-__global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
+__global__ void __launch_bounds__(FT_THREADS, 3) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
                                                                  const float *__restrict__ vol, float *__restrict__ proj,
                                                                  float margin, int bfs, int bss, int bzz, DevErr err) {
@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // a warp covers 8(u) x 4(v) pixels: <= 10 columns of the fast axis, <= 2 rows, <= 2 z-planes
     const int tu = (warp & 1) * 8 + (lane & 7), tv = (warp >> 1) * 4 + (lane >> 3);
-    const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = blockIdx.z;
+    const int iu = blockIdx.x * FT_TU + tu, iv = blockIdx.y * FT_TV + tv, view = g.view_order[blockIdx.z];
     const bool valid = iu < g.nu && iv < g.nv;
 
     // orientation: the detector u-axis is e_u = (-sin, cos); the fast shared-memory axis follows it
@@ -187,6 +187,7 @@ __global__ void __launch_bounds__(FT_THREADS) forward_tma_kernel(DevGeom g, cons
                             unpack2(fma2(wZ, sub2(b1, b0), b0), cA, cB);
                             part += cA;
                             part += cB;
+                            if (CBCT_FAULT(16)) part += 1e-3f;      // test build only: a packed stream that is NOT the scalar one
                         }
                         if (j < n) {                                                                   // odd count: the last sample alone
                             jf = (float)j;

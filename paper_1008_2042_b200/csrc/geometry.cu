@@ -1,5 +1,6 @@
 // geometry.cu -- status plumbing, geometry handle, host-buffer entry points.
 // cbct_geometry_create / _info: include/cbct.h; conventions of SURVEY.md §8(c) c.1-c.2.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -137,10 +138,10 @@ extern "C" int cbct_profile_end(double ms[2], int count[2]) {
 }
 
 // The selection variables of include/cbct.h, read once per cbct_geometry_create.  -1 = not forced.
-// Defaults: the variants that have passed the device parity suite (tests/test_gpu_projectors.py).
+// The instruction stream / lane layout of the TMA kernels, when not forced, is decided by fast_variants_ok() below.
 struct Options { int fw_impl, bp_impl, fw_packed, bt_packed, bt_lanes; };
 static Options read_options() {
-    Options o{-1, -1, CBCT_DEFAULT_FW_PACKED, CBCT_DEFAULT_BT_PACKED, CBCT_DEFAULT_BT_LANES};
+    Options o{-1, -1, -1, -1, -1};
     if (const char *e = getenv("CBCT_FORWARD_IMPL")) {
         if (!strcmp(e, "tma")) o.fw_impl = FW_TMA; else if (!strcmp(e, "tiled")) o.fw_impl = FW_TILED; else if (!strcmp(e, "global")) o.fw_impl = FW_GLOBAL;
     }
@@ -173,12 +174,93 @@ static int validate(const cbct_geometry_desc *d, double *R_out, double *step_out
     return CBCT_OK;
 }
 
+static int create_with_options(const cbct_geometry_desc *desc, Options opt, cbct_geometry **out);
+
+// ---- self-check of the fast TMA kernel variants (once per process, on the device in use) ------------------------------
+// The packed-pair instruction streams (FFMA2 / FADD2 with per-instruction rounding modes) and the skewed 8x4 lane layout
+// with same-cell merging are the fast variants of P and P^T; the scalar streams and the 16x2 layout are the plain ones.
+// Both are the same arithmetic (P: bit-identical by construction; P^T: the same integer sums up to the rounding of the
+// weight products).  Before a handle defaults to the fast variants, they are run once against the plain ones on a
+// small built-in problem (64x64x16 volume, 8 views in all four quadrants, 96x32 detector): P must agree bit for bit,
+// P^T to 2e-6 relative L2, and no device error word may be raised.  If not, every handle of this process uses the plain
+// variants and cbct_geometry_describe says so.  (Forcing a variant with CBCT_FW_PACKED / CBCT_BT_PACKED / CBCT_BT_LANES
+// bypasses the check: that is what the parity tests do to test each variant on its own.)
+static int g_fast_state = -1;                          // -1 not run, 0 rejected, 1 accepted
+static std::mutex g_fast_mu;
+static bool run_fast_selfcheck() {
+    const int nx = 64, ny = 64, nz = 16, nu = 96, nv = 32, nvw = 8;
+    const double ang[nvw] = {0.1, 0.9, 1.7, 2.5, 3.3, 4.1, 4.9, 5.7};
+    cbct_geometry_desc d{};
+    d.nx = nx; d.ny = ny; d.nz = nz; d.dx = d.dy = d.dz = 4.0; d.ox = 3.0; d.oy = -2.0; d.oz = 1.0;
+    d.nu = nu; d.nv = nv; d.du = d.dv = 3.2; d.u0 = 1.1; d.v0 = -0.7; d.sad = 1000.0; d.sdd = 1500.0;
+    d.n_views = nvw; d.angles = ang; d.step_mm = 0.0;
+    const size_t n_vox = (size_t)nx * ny * nz, n_rays = (size_t)nu * nv * nvw;
+    std::vector<float> hv(n_vox), hp(n_rays), out[4];
+    unsigned lcg = 12345u;
+    auto rnd = [&]() { lcg = lcg * 1664525u + 1013904223u; return (float)(lcg >> 8) * (1.0f / 16777216.0f); };
+    for (auto &v : hv) v = rnd();
+    for (auto &v : hp) v = rnd() - 0.4f;
+    float *d_v = nullptr, *d_p = nullptr, *d_o = nullptr;
+    bool ok = cudaMalloc(&d_v, sizeof(float) * n_vox) == cudaSuccess && cudaMalloc(&d_p, sizeof(float) * n_rays) == cudaSuccess &&
+              cudaMalloc(&d_o, sizeof(float) * std::max(n_vox, n_rays)) == cudaSuccess;
+    ok = ok && cudaMemcpy(d_v, hv.data(), sizeof(float) * n_vox, cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(d_p, hp.data(), sizeof(float) * n_rays, cudaMemcpyHostToDevice) == cudaSuccess;
+    for (int fast = 0; fast < 2 && ok; ++fast) {
+        cbct_geometry *G = nullptr;
+        ok = create_with_options(&d, Options{FW_TMA, BP_SCATTER, fast, fast, fast ? 0 : 1}, &G) == CBCT_OK;
+        if (!ok) break;
+        out[2 * fast].resize(n_rays); out[2 * fast + 1].resize(n_vox);
+        ok = launch_forward(G, d_v, d_o, nullptr) == CBCT_OK &&
+             cudaMemcpy(out[2 * fast].data(), d_o, sizeof(float) * n_rays, cudaMemcpyDeviceToHost) == cudaSuccess &&
+             launch_backproject(G, d_p, d_o, nullptr) == CBCT_OK &&
+             cudaMemcpy(out[2 * fast + 1].data(), d_o, sizeof(float) * n_vox, cudaMemcpyDeviceToHost) == cudaSuccess;
+        int bits = 0;
+        ok = ok && cbct_geometry_status(G, nullptr, &bits, 0) == CBCT_OK;
+        cbct_geometry_destroy(G);
+    }
+    cudaFree(d_v); cudaFree(d_p); cudaFree(d_o);
+    (void)cudaGetLastError();
+    if (!ok) return false;
+    if (std::memcmp(out[0].data(), out[2].data(), sizeof(float) * n_rays) != 0) return false;     // P: bit for bit
+    double num = 0, den = 0;
+    for (size_t i = 0; i < n_vox; ++i) {
+        const double a = out[1][i], b = out[3][i];
+        num += (a - b) * (a - b); den += a * a;
+    }
+    return den > 0 && num <= 4e-12 * den;                                                       // P^T: 2e-6 relative L2
+}
+#ifdef CBCT_TEST_FAULTS
+extern "C" void cbct_test_reset_selfcheck(void) { std::lock_guard<std::mutex> lk(g_fast_mu); g_fast_state = -1; }   // test build only
+#endif
+static bool fast_variants_ok() {
+    std::lock_guard<std::mutex> lk(g_fast_mu);
+    if (g_fast_state < 0) {
+        g_fast_state = 0;                              // a nested create (the check's own handles) never re-enters
+        g_fast_state = run_fast_selfcheck() ? 1 : 0;
+    }
+    return g_fast_state == 1;
+}
+
 extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometry **out) {
     if (!out) return CBCT_E_INVALID;
     *out = nullptr;
     double R = 0, step = 0;
     CBCT_TRY(validate(desc, &R, &step));
     CBCT_TRY(device_supported());
+    Options opt = read_options();
+    if (opt.fw_packed < 0 || opt.bt_packed < 0 || opt.bt_lanes < 0) {
+        const bool fast = fast_variants_ok();
+        if (opt.fw_packed < 0) opt.fw_packed = fast ? 1 : 0;
+        if (opt.bt_packed < 0) opt.bt_packed = fast ? 1 : 0;
+        if (opt.bt_lanes < 0) opt.bt_lanes = fast ? 0 : 1;
+    }
+    return create_with_options(desc, opt, out);
+}
+
+static int create_with_options(const cbct_geometry_desc *desc, Options opt, cbct_geometry **out) {
+    *out = nullptr;
+    double R = 0, step = 0;
+    CBCT_TRY(validate(desc, &R, &step));
     cbct_geometry *G = new (std::nothrow) cbct_geometry();
     if (!G) return CBCT_E_INVALID;
     G->desc = *desc;
@@ -189,6 +271,7 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     G->K = (int32_t)std::ceil(2.0 * R / step);
     G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
+    G->d_view_order = nullptr;
     G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr; G->d_fw_volT = nullptr; G->fw_tma_ok = 0;
     G->err = DevErr{nullptr, nullptr}; G->h_err = nullptr;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
@@ -198,8 +281,14 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
 
     std::vector<double2> cs(desc->n_views);
     for (int i = 0; i < desc->n_views; ++i) cs[i] = make_double2(std::cos(desc->angles[i]), std::sin(desc->angles[i]));
+    std::vector<int> order;                                    // x-fast views, then y-fast views (same rule as the kernels)
+    for (int pass = 0; pass < 2; ++pass)
+        for (int i = 0; i < desc->n_views; ++i)
+            if ((std::fabs(cs[i].x) > std::fabs(cs[i].y)) == (pass == 1)) order.push_back(i);
     cudaError_t e = cudaMalloc(&G->d_view_cs, sizeof(double2) * cs.size());
     if (e == cudaSuccess) e = cudaMemcpy(G->d_view_cs, cs.data(), sizeof(double2) * cs.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&G->d_view_order, sizeof(int) * order.size());
+    if (e == cudaSuccess) e = cudaMemcpy(G->d_view_order, order.data(), sizeof(int) * order.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&G->d_ws_vol, sizeof(float) * G->n_vox);
     if (e == cudaSuccess) e = cudaMalloc(&G->d_ws_proj, sizeof(float) * G->n_rays);
     // device error word: a device int the kernels OR into, and a mapped pinned host int the entry points poll
@@ -223,9 +312,9 @@ extern "C" int cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometr
     g.step = step;
     g.tau0 = G->t_min + 0.5 * step - desc->sad;
     g.view_cs = G->d_view_cs;
+    g.view_order = G->d_view_order;
 
     // ---- which kernels serve this handle: plan + the selection variables, read HERE and nowhere else (cbct.h) ----
-    const Options opt = read_options();
     G->fw_packed = opt.fw_packed; G->bt_packed = opt.bt_packed; G->bt_lm = opt.bt_lanes;
     plan_forward_tma(G);
     plan_backproject_tma(G);
@@ -299,7 +388,8 @@ extern "C" int cbct_geometry_describe(const cbct_geometry *G, char *buf, size_t 
     else snprintf(fw, sizeof fw, "%s", G->fw_impl == FW_TILED ? "forward_tiled_kernel" : "forward_global_kernel");
     if (G->bp_impl == BP_SCATTER) describe_backproject_tma(G, bp, sizeof bp);
     else snprintf(bp, sizeof bp, "%s", G->bp_impl == BP_CELL ? "backproject_cell_kernel + backproject_combine_kernel" : "backproject_gather_kernel");
-    snprintf(buf, cap, "forward: %s; backproject: %s", fw, bp);
+    snprintf(buf, cap, "forward: %s; backproject: %s%s", fw, bp,
+             g_fast_state == 0 ? " (fast variants rejected by the create-time self-check)" : "");
     return CBCT_OK;
 }
 
@@ -322,6 +412,7 @@ extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     cudaFree(G->err.dev);
     if (G->h_err) cudaFreeHost(G->h_err);
     cudaFree(G->d_view_cs);
+    cudaFree(G->d_view_order);
     cudaFree(G->d_ws_vol);
     cudaFree(G->d_ws_proj);
     free_bp_tables(G);

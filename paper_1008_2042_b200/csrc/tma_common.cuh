@@ -30,7 +30,7 @@ constexpr unsigned long long CBCT_WAIT_NS = 200ull * 1000ull * 1000ull;      // 
 // the product build never does, CBCT_FAULT(..) is the constant 0 there): they prove that the guards above turn a wrong
 // transaction count / a mis-planned box into an error status instead of a hang / an out-of-range access.
 #ifdef CBCT_TEST_FAULTS
-extern "C" int cbct_test_fault;      // 1: expect_tx announces 16 bytes too many; 2: forward box origin shifted; 4: scatter box origin shifted
+extern "C" int cbct_test_fault;      // 1: expect_tx announces 16 bytes too many; 2 / 4: forward / scatter box origin shifted; 8: head-room plan ignored; 16: packed forward stream perturbed
 #define CBCT_FAULT(bit) (cbct_test_fault & (bit))
 #else
 #define CBCT_FAULT(bit) 0

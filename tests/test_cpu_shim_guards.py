@@ -110,6 +110,52 @@ def test_scatter_box_that_misses_its_samples_is_reported_not_written(monkeypatch
     assert rel_l2(h.backproject(y), op.back_scatter(G, y.astype(np.float64))) <= 1e-5
 
 
+def test_exhausted_fixed_point_headroom_is_reported(monkeypatch):
+    """cbct_backproject plans its int32 accumulators for half their range; the conversion pass reports any sum that
+    reaches 2^30.  Fault 8 makes the launcher ignore the plan (all 40 views of cfg 2 in one group instead of 13 at a
+    time): P^T of all-ones then peaks above 2^30 but still below 2^31, so the volume is still right, and the word is raised."""
+    monkeypatch.setenv("CBCT_BACKPROJECT_IMPL", "scatter")
+    Gt = syn.workload(2).geometry
+    qb, group, _w = cb.backproject_fixed_point_plan(Gt)
+    assert group < Gt.n_views
+    h = sl.Geometry(Gt)
+    ones = np.ones(Gt.proj_shape, np.float32)
+    ref = op.back_scatter(Gt, ones.astype(np.float64))
+    assert rel_l2(h.backproject(ones), ref) <= 1e-5
+    assert h.status() == (cb.CBCT_OK, 0)                       # the plan holds: nothing reported
+    fault_word().value = 8
+    status, out = _raw(h, "cbct_backproject", ones, h.vol_shape)
+    fault_word().value = 0
+    assert status == cb.CBCT_OK
+    code, flags = h.status(clear=True)
+    assert code == cb.CBCT_E_DEVICE and flags == 8
+    assert 2.0 ** 30 <= ref.max() / Gt.step * 2.0 ** qb < 2.0 ** 31            # the case is what the docstring says
+    assert rel_l2(out.numpy(), ref) <= 1e-5
+
+
+def test_fast_variants_are_default_only_after_the_create_time_self_check():
+    """Unforced handles use the packed instruction streams and the skewed lane layout only if, once per process, they
+    reproduce the plain variants on a built-in problem (P bit for bit, P^T to 2e-6).  A packed stream that computes
+    something else (fault 16) is rejected: handles fall back to the plain variants and say so."""
+    L = sl.lib()
+    L.cbct_test_reset_selfcheck()
+    h = sl.Geometry(G)
+    d = h.describe()
+    assert "forward_tma_kernel<" in d and ",packed>" in d and "LM0,packed>" in d and "rejected" not in d, d
+    x = syn.uniform_volume(G, 12)
+    assert rel_l2(h.forward(x), op.forward(G, x.astype(np.float64))) <= 1e-5
+    sl.kernel_log()
+    L.cbct_test_reset_selfcheck()
+    fault_word().value = 16
+    h = sl.Geometry(G)                                        # the self-check runs here, with the broken packed stream
+    fault_word().value = 0
+    d = h.describe()
+    assert ",scalar>" in d and "LM1,scalar>" in d and "rejected by the create-time self-check" in d, d
+    assert rel_l2(h.forward(x), op.forward(G, x.astype(np.float64))) <= 1e-5
+    L.cbct_test_reset_selfcheck()                             # leave the process in its normal state
+    assert "rejected" not in sl.Geometry(G).describe()
+
+
 def test_describe_names_the_kernels_and_forced_implementations_fail_loudly(monkeypatch):
     d = sl.Geometry(G).describe()
     assert "forward_tma_kernel<" in d and "backproject_scatter_kernel<" in d
