@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 4]
     python bench.py --kernels-only      # P, P^T, fused TF, Siddon pair a few times (the command ncu wraps)
-    python bench.py --peaks             # cbct_microbench: the per-SM rates that bound P / P^T on this device
+    python bench.py --peaks             # cbct_microbench alone: the per-SM rates that bound P / P^T on this device
 
 A *step* is one pass of the whole hot path (every row) over one batch of synthetic
 input at BASELINE.json's paper-size config (512x512x70 volume, 40 views of 512x384, step 0.25 mm):
@@ -16,6 +16,13 @@ input at BASELINE.json's paper-size config (512x512x70 volume, 40 views of 512x3
 algorithmic sample count of cbct_geometry_info), inputs resident in HBM.  `e2e` = the same step driven
 through cbct_recon_run_host with HOST buffers (H2D of g, D2H of f inside the timed region).
 Multi-GPU: the path does not shard (north_star: one GPU) -> N independent replicas, weak scaling.
+
+Everything in the `roofline` object can be recomputed from the line itself: `launch_ms` is the mean CUDA-event time of the
+dominant projector inside the timed steps (events recorded by the library on the launching stream), `samples_per_launch`
+the algorithmic sample count, and the two ceilings of SURVEY.md §8(d) -- shared-memory wavefronts (8 per warp-sample) and
+thread-instruction issue (40 per sample) -- are formed from rates that cbct_microbench measures IN THIS PROCESS (conflict-
+free LDS / ATOMS wavefronts and FFMA issue per clock per SM) times the SM clock sampled during the timed region.
+`traffic` is null: it may only come from an ncu capture of the kernels now timed, and none exists for this build.
 """
 from __future__ import annotations
 
@@ -37,10 +44,11 @@ METRIC = "P+P^T projector throughput over one A2 outer iteration + TF + MG at 51
 UNIT = "Gsamples/s"
 N_CGLS = 3
 MU = 5e-4
-# algorithmic thread-instructions per trilinear sample (DESIGN.md §Roofline): 3 position FMAs, 3 floor,
+# algorithmic thread-instructions per trilinear sample (DESIGN.md §5): 3 position FMAs, 3 floor,
 # 3 frac, 3 address, 8 loads, 14 lerp ops, 1 accumulate, ~5 loop/convert = 40
 INSTR_PER_SAMPLE = 40.0
-N_SM, LANES_PER_CLK_PER_SM = 148, 128
+ACCESSES_PER_SAMPLE = 8.0          # shared-memory loads (P) / integer reductions (P^T) per sample: 8 wavefronts per warp-sample
+N_SM, SMSP_PER_SM = 148, 4
 
 
 def load_peaks():
@@ -154,6 +162,7 @@ def main():
     ap.add_argument("--kernels-only", action="store_true", help="run P, P^T, fused TF 3x and exit (for ncu)")
     ap.add_argument("--peaks", action="store_true", help="run the library's micro-benchmarks (cbct_microbench) and exit")
     ap.add_argument("--no-full-recon", action="store_true", help="skip the one-off 3-level 5/10/15 reconstruction timing")
+    ap.add_argument("--no-variants", action="store_true", help="skip the A/B timings of the other kernel variants")
     args = ap.parse_args()
 
     from paper_1008_2042_b200 import replicas
@@ -182,16 +191,13 @@ def main():
     if w.photons:
         g = syn.add_poisson_noise(g, w.photons, w.seed + rank)          # every replica its own noise draw
 
-    if args.peaks:
-        # per-SM rates that bound P / P^T; rates per clock are converted with the max SM clock for context
+    def measure_peaks():
+        """per-SM rates of cbct_microbench; per-clock rates need no clock assumption"""
         res = cb.microbench()
-        clk = load_peaks()["sm_max_mhz"] * 1e6
-        line = dict(peaks=True, n_sm=N_SM, sm_max_mhz=clk / 1e6)
-        for name, (rate, unit) in res.items():
-            line[name] = dict(value=rate, unit=unit)
-        line["derived"] = dict(
-            ffma_tinstr_s=res["ffma"][0] * 32 * N_SM * clk / 1e12, ffma2_tinstr_s=res["ffma2"][0] * 64 * N_SM * clk / 1e12,
-            lds_wavefronts_per_clk_sm=res["lds32"][0], atoms_wavefronts_per_clk_sm=res["atoms_add_s32"][0])
+        return {name: dict(value=rate, unit=unit) for name, (rate, unit) in res.items()}
+
+    if args.peaks:
+        line = dict(peaks=True, n_sm=N_SM, **measure_peaks())
         os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
         with open(os.path.join(ROOT, "gpurun_out", "peaks_local.json"), "w") as fh:
             json.dump(line, fh, indent=1)
@@ -219,11 +225,15 @@ def main():
         s[1].record(); geom.siddon_backproject(d_g, d_out)
         s[2].record()
         torch.cuda.synchronize()
+        ok, bits = geom.status()
         e = evs[-1]
-        print(json.dumps(dict(kernels_only=True, workload=args.workload, p_ms=e[0].elapsed_time(e[1]),
+        print(json.dumps(dict(kernels_only=True, workload=args.workload, kernels=geom.describe(), device_status=bits,
+                              p_ms=e[0].elapsed_time(e[1]),
                               pt_ms=e[1].elapsed_time(e[2]), tf_fused_ms=e[2].elapsed_time(e[3]),
                               siddon_p_ms=s[0].elapsed_time(s[1]), siddon_pt_ms=s[1].elapsed_time(s[2]),
                               samples=geom.n_samples)), flush=True)
+        if not ok:
+            raise SystemExit(3)
         return
 
     geom = cb.Geometry(G)                                                 # for the standalone P / P^T timing
@@ -285,6 +295,7 @@ def main():
     clocks = sampler.stop() if sampler else None
     step_ms = replicas.max_over_ranks(float(np.sum(ms)), "cuda")
     value = world * samples_per_step * args.steps / (step_ms * 1e-3) / 1e9
+    rec_ok, rec_bits = rec.status()
 
     # ---- end-to-end arm (host buffers through the C ABI) -----------------------------------------
     for _ in range(2):
@@ -295,77 +306,164 @@ def main():
     e2e_ms = replicas.max_over_ranks(float(np.sum(ms_e2e)), "cuda")
     e2e_value = world * samples_per_step * args.steps / (e2e_ms * 1e-3) / 1e9
 
-    # ---- standalone kernels (context numbers) -----------------------------------------------------
-    d_vol = torch.from_numpy(f0).cuda()
-    d_proj = torch.empty(geom.proj_shape, dtype=torch.float32, device="cuda")
-    for _ in range(3):
-        geom.forward(d_vol, d_proj); geom.backproject(d_g, d_tmp)
-    ms_p = float(np.median(timed(lambda: geom.forward(d_vol, d_proj), 5)))
-    ms_pt = float(np.median(timed(lambda: geom.backproject(d_g, d_tmp), 5)))
-    ms_tf = float(np.median(timed(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True), 5)))
-    # the paper's own pair (Siddon) and the scalar instruction stream of P: context numbers
-    geom.siddon_forward(d_vol, d_proj); geom.siddon_backproject(d_g, d_tmp)
-    ms_sp = float(np.median(timed(lambda: geom.siddon_forward(d_vol, d_proj), 3)))
-    ms_spt = float(np.median(timed(lambda: geom.siddon_backproject(d_g, d_tmp), 3)))
-    os.environ["CBCT_FW_PACKED"] = "0"
-    geom.forward(d_vol, d_proj)
-    ms_p_scalar = float(np.median(timed(lambda: geom.forward(d_vol, d_proj), 5)))
-    del os.environ["CBCT_FW_PACKED"]
-
-    # ---- the paper's full reconstruction, end to end (context number; 3 levels, 5/10/15) ----
-    full_recon_s = None
-    if rank == 0 and not args.no_full_recon:
-        del d_alpha                                            # 2 GB of three-call coefficients no longer needed
-        rec3 = cb.Recon(G, 3)
-        rec3.run(d_g, d_f, [1, 1, 1], N_CGLS, MU, True)       # warm-up
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        rec3.run(d_g, d_f, [5, 10, 15], N_CGLS, MU, True)
-        b.record()
-        torch.cuda.synchronize()
-        full_recon_s = a.elapsed_time(b) * 1e-3
-        rrms = float(torch.linalg.vector_norm(d_f - d_vol) / torch.linalg.vector_norm(d_vol))
-        rec3.close()
-
     if rank != 0:
         replicas.shutdown()
         return
 
-    peaks = load_peaks()
-    # dominant kernel = the projector with the larger share of the step
+    errors = []
+
+    def guarded(what, fn, default=None):
+        """context numbers must never cost the bench line: a failure is recorded, not raised"""
+        try:
+            return fn()
+        except Exception as exc:  # noqa: BLE001
+            errors.append(f"{what}: {type(exc).__name__}: {exc}")
+            return default
+
+    # ---- standalone kernels (the headline's components) -------------------------------------------------
+    d_vol = torch.from_numpy(f0).cuda()
+    d_proj = torch.empty(geom.proj_shape, dtype=torch.float32, device="cuda")
+
+    def med(fn, n=5):
+        fn()
+        return float(np.median(timed(fn, n)))
+
+    ms_p = med(lambda: geom.forward(d_vol, d_proj))
+    ms_pt = med(lambda: geom.backproject(d_g, d_tmp))
+    ms_tf = med(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True))
+    geom_ok, geom_bits = geom.status()
+
+    # ---- roofline denominators, measured in this process (SURVEY.md §8(d)) -------------------------------------
+    peaks = guarded("cbct_microbench", measure_peaks, {})
+    hbm = load_peaks()
+    f_clk_mhz = (clocks or {}).get("sm_mhz") or hbm["sm_max_mhz"]
+    f_clk = f_clk_mhz * 1e6
+
+    def rate(name, nominal):
+        v = (peaks.get(name) or {}).get("value")
+        return (float(v), "measured (cbct_microbench, this process)") if v else (nominal, "nominal (micro-benchmark unavailable)")
+
     (ms_f, n_f), (ms_b, n_b) = prof["forward"], prof["backproject"]
-    dom = "backproject" if ms_b >= ms_f else "forward"
-    dom_ms = (ms_b / max(n_b, 1)) if dom == "backproject" else (ms_f / max(n_f, 1))
-    f_clk = peaks["sm_max_mhz"] * 1e6
-    peak_tinstr = N_SM * LANES_PER_CLK_PER_SM * f_clk / 1e12
-    achieved_tinstr = geom.n_samples * INSTR_PER_SAMPLE / (dom_ms * 1e-3) / 1e12
-    # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` captures (profiles/README.md),
-    # cfg 4 only: P = forward_tma_kernel (r1_kernels_full.csv), P^T = scatter kernel, both view groups (r1_scatter_full.csv)
-    ncu_traffic = {("forward", 4): 1.851507e9 + 35.917e6, ("backproject", 4): (439.53e6 + 84.42e6) + (2.635912e9 + 0.169432e9)}
-    roofline = dict(bound="alu", kernel=f"cbct_{dom}", achieved=achieved_tinstr, peak=peak_tinstr, unit="Tinstr/s",
-                    frac=achieved_tinstr / peak_tinstr, traffic=ncu_traffic.get((dom, args.workload)),
-                    traffic_unit="DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum); algorithmic HBM bytes "
-                                 "are 105e6 per launch, the kernel is not HBM bound; taken from the committed r1 captures (scalar streams, "
-                                 "16x2 scatter layout) -- the packed default kernels move the same data and are to be re-captured",
-                    algorithmic=f"{geom.n_samples} samples x {INSTR_PER_SAMPLE:.0f} thread-instr/sample per launch",
-                    launch_ms=dom_ms, gsamples_s=geom.n_samples / (dom_ms * 1e-3) / 1e9,
-                    peak_source=f"148 SM x 128 lanes/clk x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)",
-                    share_of_step=dict(forward=ms_f / step_ms, backproject=ms_b / step_ms))
+    per_call = dict(forward=ms_f / max(n_f, 1), backproject=ms_b / max(n_b, 1))
+    dom = "backproject" if per_call["backproject"] >= per_call["forward"] else "forward"
+    wave_name = "atoms_add_s32" if dom == "backproject" else "lds32"
+    r_wave, src_wave = rate(wave_name, 1.0)               # conflict-free warp instructions (= wavefronts) per clock per SM
+    r_issue, src_issue = rate("ffma", float(SMSP_PER_SM))  # warp instructions issued per clock per SM
+
+    def ceilings(r_w, r_i):
+        return dict(lsu_wavefront=N_SM * r_w * f_clk * 32.0 / ACCESSES_PER_SAMPLE / 1e9,
+                    thread_instr=N_SM * r_i * f_clk * 32.0 / INSTR_PER_SAMPLE / 1e9)
+
+    ceil = ceilings(r_wave, r_issue)
+    binding = min(ceil, key=ceil.get)
+    dom_ms = per_call[dom]
+    achieved = geom.n_samples / (dom_ms * 1e-3) / 1e9
+    roofline = dict(
+        bound="alu", kernel=f"cbct_{dom}", kernels=geom.describe(), achieved=achieved, peak=ceil[binding], unit="Gsamples/s",
+        frac=achieved / ceil[binding], binding=binding, traffic=None,
+        traffic_note="null: no ncu capture of the kernels timed here exists (GPU use was closed to this repository while they "
+                     "were written); algorithmic HBM bytes are 105e6 per launch = 16 us, the projectors are not HBM bound",
+        launch_ms=dom_ms, samples_per_launch=geom.n_samples,
+        ceilings_gsamples_s=ceil,
+        frac_lsu_wavefront=achieved / ceil["lsu_wavefront"], frac_thread_instr=achieved / ceil["thread_instr"],
+        formula="lsu_wavefront = 148 SM x wavefronts/clk/SM x f_clk x 32 lanes / 8 accesses per sample; "
+                "thread_instr = 148 SM x warp-instr/clk/SM x f_clk x 32 lanes / 40 instructions per sample; peak = the lower",
+        rates=dict(wavefronts_per_clk_per_sm=r_wave, wavefront_kind=wave_name, wavefront_source=src_wave,
+                   warp_instr_per_clk_per_sm=r_issue, issue_source=src_issue, sm_clock_mhz=f_clk_mhz,
+                   sm_clock_source="median nvidia-smi clocks.sm during the timed region" if (clocks or {}).get("sm_mhz") else "max SM clock"),
+        other_projector=dict(kernel="cbct_forward" if dom == "backproject" else "cbct_backproject",
+                             launch_ms=per_call["forward" if dom == "backproject" else "backproject"]),
+        share_of_step=dict(forward=ms_f / step_ms, backproject=ms_b / step_ms))
+    for k in ("forward", "backproject"):                  # both §8(d) fractions for both projectors
+        a = geom.n_samples / (per_call[k] * 1e-3) / 1e9
+        rw, _ = rate("atoms_add_s32" if k == "backproject" else "lds32", 1.0)
+        c = ceilings(rw, r_issue)
+        roofline[f"{k}_gsamples_s"] = a
+        roofline[f"{k}_frac"] = dict(lsu_wavefront=a / c["lsu_wavefront"], thread_instr=a / c["thread_instr"], binding=min(c, key=c.get))
+
+    # ---- A/B timings of the other kernel variants (context; each variant is a handle created under its selection variable) ----
+    variants = {}
+    if not args.no_variants:
+        sel = ("CBCT_FORWARD_IMPL", "CBCT_BACKPROJECT_IMPL", "CBCT_FW_PACKED", "CBCT_BT_PACKED", "CBCT_BT_LANES")
+
+        def variant(env, fn_name, src, dst):
+            saved = {k: os.environ.pop(k, None) for k in sel}
+            os.environ.update(env)
+            try:
+                h = cb.Geometry(G)
+            finally:
+                for k in sel:
+                    os.environ.pop(k, None)
+                    if saved[k] is not None:
+                        os.environ[k] = saved[k]
+            t = med(lambda: getattr(h, fn_name)(src, dst), 3)
+            ok, bits = h.status()
+            d = h.describe()
+            h.close()
+            return dict(ms=t, kernel=d.split("; ")[0 if fn_name == "forward" else 1], device_status=bits)
+
+        for name, env in (("p_tma_scalar", {"CBCT_FORWARD_IMPL": "tma", "CBCT_FW_PACKED": "0"}),
+                          ("p_tma_packed", {"CBCT_FORWARD_IMPL": "tma", "CBCT_FW_PACKED": "1"}),
+                          ("p_tiled", {"CBCT_FORWARD_IMPL": "tiled"})):
+            variants[name] = guarded(name, lambda env=env: variant(env, "forward", d_vol, d_proj))
+        for name, env in (("pt_scatter_lm1_scalar", {"CBCT_BACKPROJECT_IMPL": "scatter", "CBCT_BT_LANES": "1", "CBCT_BT_PACKED": "0"}),
+                          ("pt_scatter_lm1_packed", {"CBCT_BACKPROJECT_IMPL": "scatter", "CBCT_BT_LANES": "1", "CBCT_BT_PACKED": "1"}),
+                          ("pt_scatter_lm0_scalar", {"CBCT_BACKPROJECT_IMPL": "scatter", "CBCT_BT_LANES": "0", "CBCT_BT_PACKED": "0"}),
+                          ("pt_scatter_lm0_packed", {"CBCT_BACKPROJECT_IMPL": "scatter", "CBCT_BT_LANES": "0", "CBCT_BT_PACKED": "1"}),
+                          ("pt_cell", {"CBCT_BACKPROJECT_IMPL": "cell"})):
+            variants[name] = guarded(name, lambda env=env: variant(env, "backproject", d_g, d_tmp))
+    # the paper's own pair (Siddon, SURVEY §8(f) NEXT-2), Eq. 3 and the HBM-bound kernels: context numbers
+    ctx = {}
+    ctx["siddon_p_ms"] = guarded("siddon_forward", lambda: med(lambda: geom.siddon_forward(d_vol, d_proj), 3))
+    ctx["siddon_pt_ms"] = guarded("siddon_backproject", lambda: med(lambda: geom.siddon_backproject(d_g, d_tmp), 3))
+    ctx["eq3_ms"] = guarded("backproject_eq3", lambda: med(lambda: geom.backproject_eq3(d_g, d_tmp), 3))
+    ctx["tf_decompose_ms"] = guarded("tf_decompose", lambda: med(lambda: cb.tf_decompose(d_vol, d_alpha), 3))
+    ctx["tf_shrink_ms"] = guarded("tf_shrink", lambda: med(lambda: cb.tf_shrink(d_alpha, MU), 3))
+    ctx["tf_reconstruct_ms"] = guarded("tf_reconstruct", lambda: med(lambda: cb.tf_reconstruct(d_alpha, d_tmp), 3))
+    ctx["tf_reconstruct_direct_ms"] = guarded("tf_reconstruct_direct", lambda: med(lambda: cb.tf_reconstruct_direct(d_alpha, d_tmp), 2))
+    ctx["mg_prolong_ms"] = guarded("mg_prolong", lambda: med(lambda: cb.mg_prolong(d_coarse, d_tmp), 3))
+    ctx["mg_restrict_ms"] = guarded("mg_restrict", lambda: med(lambda: cb.mg_restrict(d_tmp, d_coarse), 3))
+
+    # ---- the paper's full reconstruction, end to end (context number; PAPER.md:288: 3 levels, 5/10/15) ----
+    full_recon_s, rrms = None, None
+    if not args.no_full_recon:
+        def full():
+            rec3 = cb.Recon(G, 3)
+            rec3.run(d_g, d_f, [1, 1, 1], N_CGLS, MU, True)       # warm-up
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            rec3.run(d_g, d_f, [5, 10, 15], N_CGLS, MU, True)
+            b.record()
+            torch.cuda.synchronize()
+            ok3, bits3 = rec3.status()
+            r = float(torch.linalg.vector_norm(d_f - d_vol) / torch.linalg.vector_norm(d_vol))
+            rec3.close()
+            if not ok3:
+                errors.append(f"full reconstruction: device error word {bits3}")
+            return a.elapsed_time(b) * 1e-3, r
+        del d_alpha                                            # 2 GB of three-call coefficients no longer needed
+        full_recon_s, rrms = guarded("full reconstruction", full, (None, None))
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        r = time_oracle_sample(G, f0, g, [0, G.n_views // 3])
+        r = time_oracle_sample(G, f0, g, [G.n_views // 3])
         cpu_baseline = dict(value=r["samples"] / r["seconds"] / 1e9, unit=UNIT, cores=omp_threads(), kind="oracle",
-                            sample=f"oracle P + P^T (fp64, scatter form) on 2 of {G.n_views} views of the same workload: "
+                            sample=f"oracle P + P^T (fp64, scatter form) on 1 of {G.n_views} views of the same workload: "
                                    f"{r['samples']:.3g} samples in {r['seconds']:.1f} s",
                             p_gsamples_s=0.5 * r["samples"] / r["t_forward"] / 1e9,
                             pt_gsamples_s=0.5 * r["samples"] / r["t_back"] / 1e9)
 
+    if not (rec_ok and geom_ok):
+        errors.append(f"device error word raised: recon {rec_bits}, geometry {geom_bits} -- the numbers of this line are INVALID")
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
         ms_per_step=step_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
         data="synthetic",
+        # BASELINE.json's metric, spelled out: P and P^T throughput, roofline fraction, seconds per CGLS iteration
+        s_per_cgls_iter=(per_call["forward"] + per_call["backproject"]) * 1e-3 + 0.0,
+        p_gsamples_s=geom.n_samples / ms_p / 1e6, pt_gsamples_s=geom.n_samples / ms_pt / 1e6,
+        kernels=geom.describe(),
         config=dict(workload=f"cfg{args.workload}:{w.name} {G.nx}x{G.ny}x{G.nz} vol ({G.dx}x{G.dy}x{G.dz} mm), "
                              f"{G.n_views}x{G.nv}x{G.nu} proj, SAD {G.sad:.0f}/SDD {G.sdd:.0f} mm",
                     step_mm=geom.step_mm, K=geom.K, samples_per_projector_call=geom.n_samples,
@@ -378,17 +476,17 @@ def main():
                  d2h_bytes_per_step=int(h_f.numel() * 4), ms_per_step=e2e_ms / args.steps,
                  api="cbct_recon_run_host (HOST g in, HOST f out) + TF/MG tail on the returned volume"),
         roofline=roofline, cpu_baseline=cpu_baseline,
-        extra=dict(p_ms=ms_p, pt_ms=ms_pt, tf_fused_ms=ms_tf, p_scalar_stream_ms=ms_p_scalar,
-                   siddon_p_ms=ms_sp, siddon_pt_ms=ms_spt,
-                   p_gsamples_s=geom.n_samples / ms_p / 1e6, pt_gsamples_s=geom.n_samples / ms_pt / 1e6,
-                   s_per_cgls_iter=(ms_p + ms_pt) * 1e-3 + 0.0,
-                   s_per_cgls_iter_in_step=(ms_f / max(n_f, 1) + ms_b / max(n_b, 1)) * 1e-3,
+        extra=dict(p_ms=ms_p, pt_ms=ms_pt, tf_fused_ms=ms_tf,
+                   s_per_cgls_iter_standalone=(ms_p + ms_pt) * 1e-3,
+                   s_per_cgls_iter_note="top-level s_per_cgls_iter = mean P + mean P^T launch time inside the timed steps "
+                                        "(vector kernels add < 2 %); standalone = the two kernels timed alone after an L2 flush",
+                   variants=variants, context_ms=ctx, microbench=peaks,
                    full_recon_s=full_recon_s,
                    full_recon="3-level multigrid, 5/10/15 A2 outer iterations, n_cgls=3, mu=5e-4, device-resident "
                               "(PAPER.md:288 recipe; paper: ~5 min on Tesla C1060)",
-                   full_recon_rrms_vs_phantom=(rrms if full_recon_s is not None else None),
-                   tf_fused_gbs=2 * geom.n_vox * 4 / ms_tf / 1e6, hbm_peak_gbs=peaks["hbm_gbs"],
-                   wall_s_timed_region=t_wall,
+                   full_recon_rrms_vs_phantom=rrms,
+                   tf_fused_gbs=2 * geom.n_vox * 4 / ms_tf / 1e6, hbm_peak_gbs=hbm["hbm_gbs"], hbm_peak_source=hbm["source"],
+                   wall_s_timed_region=t_wall, errors=errors,
                    paper_context="paper: ~2.7-3.5 s per P+P^T pair, ~5 min full recon on Tesla C1060 (PAPER.md:23, :402)"))
     print(json.dumps(line), flush=True)
     replicas.shutdown()

@@ -245,7 +245,13 @@ int cbct_recon_run(cbct_recon *recon, const float *d_g, float *d_f, const int *n
 int cbct_recon_run_host(cbct_recon *recon, const float *h_g, float *h_f, const int *n_outer, int n_cgls,
                         float mu, int momentum, void *stream);
 
-/* One-shot convenience wrappers: create + run + synchronise + destroy. */
+/* Device error words of the per-level geometry handles, ORed (cbct_geometry_status); synchronises `stream`. */
+int cbct_recon_status(cbct_recon *recon, void *stream, int *flags, int clear);
+/* The kernels serving the finest level (cbct_geometry_describe). */
+int cbct_recon_describe(const cbct_recon *recon, char *buf, size_t cap);
+
+/* One-shot convenience wrappers: create + run + synchronise + destroy.  A raised device error word is returned as
+ * CBCT_E_DEVICE. */
 int cbct_tf_reconstruct(const cbct_geometry_desc *finest, const float *d_g, float *d_f, int n_levels,
                         const int *n_outer, int n_cgls, float mu, int momentum, void *stream);
 /* Same with HOST buffers: copies h_g to the device, reconstructs, copies the volume back to h_f. */

@@ -29,7 +29,7 @@ EXPORTS = [
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
-    "cbct_recon_create", "cbct_recon_destroy", "cbct_recon_run", "cbct_recon_run_host",
+    "cbct_recon_create", "cbct_recon_destroy", "cbct_recon_run", "cbct_recon_run_host", "cbct_recon_status", "cbct_recon_describe",
     "cbct_tf_reconstruct", "cbct_tf_reconstruct_host",
 ]
 
@@ -111,6 +111,8 @@ def _declare(L):
     L.cbct_recon_destroy.argtypes = [vp]
     L.cbct_recon_run.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
     L.cbct_recon_run_host.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
+    L.cbct_recon_status.argtypes = [vp, vp, C.POINTER(C.c_int), ip]
+    L.cbct_recon_describe.argtypes = [vp, C.c_char_p, C.c_size_t]
     L.cbct_tf_reconstruct.argtypes = [C.POINTER(GeometryDesc), fp, fp, ip, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
     L.cbct_tf_reconstruct_host.argtypes = [C.POINTER(GeometryDesc), fp, fp, ip, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
     for name in EXPORTS:
@@ -424,6 +426,19 @@ class Recon:
             self.close()
         except Exception:      # interpreter shutdown: module globals may already be gone
             pass
+
+    def status(self, clear: bool = False, stream=None):
+        """(ok, [raised CBCT_STATUS_* bits]) over all levels; synchronises the stream (cbct_recon_status)"""
+        flags = C.c_int(0)
+        s = lib().cbct_recon_status(self.handle, _stream(stream), C.byref(flags), int(clear))
+        if s not in (CBCT_OK, CBCT_E_DEVICE):
+            raise CbctError(s, "cbct_recon_status")
+        return s == CBCT_OK, [n for b, n in STATUS_BITS.items() if flags.value & b]
+
+    def describe(self) -> str:
+        buf = C.create_string_buffer(512)
+        _check(lib().cbct_recon_describe(self.handle, buf, len(buf)), "cbct_recon_describe")
+        return buf.value.decode()
 
     def _outer(self, n_outer: Sequence[int]):
         assert len(n_outer) == self.n_levels

@@ -123,15 +123,31 @@ extern "C" int cbct_recon_run_host(cbct_recon *R, const float *h_g, float *h_f, 
     return CBCT_OK;
 }
 
+extern "C" int cbct_recon_status(cbct_recon *R, void *stream, int *flags, int clear) {
+    if (!R) return CBCT_E_INVALID;
+    int all = 0, status = CBCT_OK;
+    for (auto &L : R->lev) {
+        int bits = 0;
+        const int s = cbct_geometry_status(L.geom, stream, &bits, clear);
+        if (s != CBCT_OK && s != CBCT_E_DEVICE) return s;
+        if (s == CBCT_E_DEVICE) status = CBCT_E_DEVICE;
+        all |= bits;
+    }
+    if (flags) *flags = all;
+    return status;
+}
+
+extern "C" int cbct_recon_describe(const cbct_recon *R, char *buf, size_t cap) {
+    if (!R || R->lev.empty()) return CBCT_E_INVALID;
+    return cbct_geometry_describe(R->lev.back().geom, buf, cap);
+}
+
 extern "C" int cbct_tf_reconstruct(const cbct_geometry_desc *finest, const float *d_g, float *d_f, int n_levels,
                                    const int *n_outer, int n_cgls, float mu, int momentum, void *stream) {
     cbct_recon *R = nullptr;
     CBCT_TRY(cbct_recon_create(finest, n_levels, &R));
     int s = cbct_recon_run(R, d_g, d_f, n_outer, n_cgls, mu, momentum, stream);
-    if (s == CBCT_OK) {
-        const cudaError_t e = cudaStreamSynchronize(as_stream(stream));
-        if (e != cudaSuccess) s = set_cuda_error(e);
-    }
+    if (s == CBCT_OK) s = cbct_recon_status(R, stream, nullptr, 0);      // synchronises; CBCT_E_DEVICE if a kernel gave up
     cbct_recon_destroy(R);
     return s;
 }
@@ -140,7 +156,8 @@ extern "C" int cbct_tf_reconstruct_host(const cbct_geometry_desc *finest, const 
                                         const int *n_outer, int n_cgls, float mu, int momentum, void *stream) {
     cbct_recon *R = nullptr;
     CBCT_TRY(cbct_recon_create(finest, n_levels, &R));
-    const int s = cbct_recon_run_host(R, h_g, h_f, n_outer, n_cgls, mu, momentum, stream);
+    int s = cbct_recon_run_host(R, h_g, h_f, n_outer, n_cgls, mu, momentum, stream);
+    if (s == CBCT_OK) s = cbct_recon_status(R, stream, nullptr, 0);
     cbct_recon_destroy(R);
     return s;
 }

@@ -1,6 +1,6 @@
 """Instruction mix of the hot loops of the projector kernels, from the SASS of the built objects (no GPU needed).
 
-    python -m paper_1008_2042_b200.sass_report            # markdown table on stdout
+    python tests/sass_report.py            # markdown table on stdout   (TEST TOOLING: tests/test_sass_budget.py is its user)
 
 For every instantiation of forward_tma_kernel / backproject_scatter_kernel / the Siddon kernels in
 paper_1008_2042_b200/build/*.o it finds the innermost loop that contains the kernel's shared-memory loads (LDS), shared
@@ -17,7 +17,7 @@ import subprocess
 import sys
 from collections import Counter
 
-HERE = os.path.dirname(os.path.abspath(__file__))
+HERE = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_1008_2042_b200")
 KERNELS = {"forward_tma_kernel": "LDS", "backproject_scatter_kernel": "ATOMS", "siddon_forward_kernel": "LDG",
            "siddon_scatter_kernel": "RED"}
 

@@ -1,6 +1,7 @@
 """Static check of what nvcc emitted for the hot loops (no GPU): the instruction counts DESIGN.md §5 and
 profiles/r1_sass_hot_loops.md quote are held here, so a source change that bloats a hot loop fails `-m "not gpu"`.
-Uses `python -m paper_1008_2042_b200.sass_report` (cuobjdump on the built objects)."""
+Uses tests/sass_report.py (cuobjdump on the built objects)."""
+import os
 import re
 import shutil
 import subprocess
@@ -16,7 +17,8 @@ def report():
     if not shutil.which("cuobjdump"):
         pytest.skip("cuobjdump not on PATH")
     cuda_build.build()
-    out = subprocess.run([sys.executable, "-m", "paper_1008_2042_b200.sass_report"], capture_output=True, text=True, check=True).stdout
+    tool = os.path.join(os.path.dirname(os.path.abspath(__file__)), "sass_report.py")
+    out = subprocess.run([sys.executable, tool], capture_output=True, text=True, check=True).stdout
     rows = {}
     for line in out.splitlines():
         m = re.match(r"\| `(?:void )?([^`]+)` \((\d+) instantiations\) \| (\d+) \| (\d+) \| ([\d.]+) \| (.*) \|", line)
