@@ -13,12 +13,15 @@
 //     by the TMA unit, which is the transpose of the forward kernel's zero fill.  Two boxes alternate, so the
 //     reduction of one chunk overlaps the scattering of the next;
 //   * a last pass converts the accumulators to fp32 (x step / scale) with coalesced float4 stores.
-// Fixed point: every ray value is scaled by S = 2^qb / max|g| (max|g| reduced on the device per call), each
-// contribution S g w is rounded to the nearest integer by one FFMA onto 1.5 * 2^23, and qb is chosen at
-// geometry-create so that the largest possible voxel sum of a view group stays below 2^31.  The rounding
-// error per contribution is uniform in +-max|g| / 2^(qb+1) (qb = 21 at the paper-size config): relative to the
-// result that is ~1e-6 * max|g| / rms(g) -- an order of magnitude below the fp32 rounding of the weights
-// themselves for any input whose peak is within ~30 rms (projections, CGLS residuals).
+// Fixed point: every ray value is scaled by S = 2^qb / T, T = min(max|g|, 8 rms(g)) (both reduced on the device per
+// call, in a fixed order), each contribution S g w is rounded to the nearest integer by one FFMA onto 1.5 * 2^23, and
+// qb is chosen at geometry-create so that the largest possible voxel sum of a view group stays below 2^30.  The
+// rounding error per contribution is uniform in +-T / 2^(qb+1) (qb = 21 at the paper-size config): relative to the
+// result at most ~5e-6 even for white noise (where the result itself is small by cancellation), ~1e-7 for projections.
+// Rays with |g| > T (outliers of a heavy-tailed input, e.g. CGLS residuals of low-count Poisson data; none for ordinary
+// projections, where max|g| < 8 rms) are left out by the scatter kernel and added by backproject_outlier_kernel with
+// their own, coarser unit T 2^m / 2^qb, 2^m >= |g| / T: the same RELATIVE precision for them, and the unit of all
+// other rays no longer grows with the single largest value.
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -117,9 +120,10 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
     rl.bf = yfast ? r.by : r.bx; rl.bs = yfast ? r.bx : r.by; rl.bz = r.bz;
 
     // ray value in fixed-point units: |gs| <= 2^qb
-    const float amax = __uint_as_float(__ldg(absmax_bits));
-    const float scale = (amax > 0.f && amax <= 3.0e38f) ? two_qb / amax : 0.f;      // non-finite max|g|: contribute nothing (finalize writes NaN)
-    const float gs = valid ? __ldg(proj + ((size_t)view * g.nv + iv) * g.nu + iu) * scale : 0.f;
+    const float amax = __uint_as_float(__ldg(absmax_bits));           // the caller passes the reference T (bt_reference_kernel)
+    const float scale = (amax > 0.f && amax <= 3.0e38f) ? two_qb / amax : 0.f;      // non-finite reference: contribute nothing (finalize writes NaN)
+    float gs = valid ? __ldg(proj + ((size_t)view * g.nv + iv) * g.nu + iu) * scale : 0.f;
+    if (!(fabsf(gs) <= two_qb)) gs = 0.f;                   // an outlier (|g| > T): backproject_outlier_kernel adds it
 
     if (tid == 0) { s_klo = 0x7fffffff; s_khi = -1; s_abort = *reinterpret_cast<volatile int *>(err.dev); }
     if ((tu == 0 || tu == FT_TU - 1) && (tv == 0 || tv == FT_TV - 1)) corner[(tv ? 2 : 0) + (tu ? 1 : 0)] = rl;
@@ -297,7 +301,85 @@ __global__ void __launch_bounds__(FT_THREADS) backproject_scatter_kernel(DevGeom
     if (tid == 0) bulk_wait0();                           // shared memory must outlive the last reduction
 }
 
-// vol[z][y][x] (+)= (acc_x[z][y][x] + acc_y[z][x][y]) * step * max|g| / 2^qb; 32x32 tiles, the y-fastest accumulator is
+// T = min(max|g|, 8 rms(g)) -> ref[1] (bits); a non-finite max|g| is passed on (the volume becomes NaN)
+__global__ void bt_reference_kernel(unsigned *ref, const double *sumsq, double n) {
+    const float amax = __uint_as_float(ref[0]);
+    float t = amax;
+    if (amax <= 3.0e38f) {
+        const float r8 = (float)(8.0 * sqrt(*sumsq / n));
+        if (r8 > 0.f && r8 < amax) t = r8;
+    }
+    ref[1] = __float_as_uint(t);
+}
+
+// The rays the scatter kernel left out (|g| > T).  A warp looks at 32 rays at a time; every outlier among them is then
+// sampled by the whole warp (lanes stride over the samples of the ray, same positions and weights as the scatter
+// kernel's direct path) and added to the x-fastest accumulator with integer atomics, each contribution rounded to a
+// multiple of 2^m units, 2^m >= |g| / T: |g S / 2^m| <= 2^qb keeps the rounding trick in range.
+__global__ void __launch_bounds__(256) backproject_outlier_kernel(DevGeom g, const float *__restrict__ proj, int *__restrict__ acc_x,
+                                                                  const unsigned *__restrict__ ref, float two_qb, int view0, int n_views,
+                                                                  int pf, int ps, int pz) {
+    const float t = __uint_as_float(__ldg(ref));
+    if (!(t > 0.f && t <= 3.0e38f)) return;
+    const float scale = two_qb / t;
+    const long long per_view = (long long)g.nv * g.nu, n = per_view * n_views;
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long base = warp0 * 32; base < n; base += n_warps * 32) {
+        const long long i = base + lane;
+        float gs = 0.f;
+        int view = 0, pix = 0;
+        if (i < n) {
+            view = g.view_order[view0 + (int)(i / per_view)];
+            pix = (int)(i % per_view);
+            gs = __ldg(proj + (size_t)view * per_view + pix) * scale;
+        }
+        unsigned todo = __ballot_sync(0xffffffffu, i < n && !(fabsf(gs) <= two_qb) && fabsf(gs) <= 3.0e38f);
+        while (todo) {
+            const int src = __ffs(todo) - 1;
+            todo &= todo - 1;
+            const float gso = __shfl_sync(0xffffffffu, gs, src);
+            const int vw = __shfl_sync(0xffffffffu, view, src), px = __shfl_sync(0xffffffffu, pix, src);
+            int m = 0;
+            float gq = gso;
+            while (fabsf(gq) > two_qb && m < 30) { gq *= 0.5f; ++m; }
+            RayF r;
+            double b[3], c[3];
+            ray_setup(g, vw, px / g.nu, px % g.nu, r, b[0], b[1], b[2], c[0], c[1], c[2]);
+            const double hi[3] = {(double)g.nx, (double)g.ny, (double)g.nz};
+            double tin = -1e300, tout = 1e300;
+            bool miss = false;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                if (b[a] == 0.0) { miss |= (c[a] <= -1.0 || c[a] >= hi[a]); continue; }
+                const double inv = 1.0 / b[a];
+                double t1 = (-1.0 - c[a]) * inv, t2 = (hi[a] - c[a]) * inv;
+                if (t1 > t2) { const double tt = t1; t1 = t2; t2 = tt; }
+                tin = fmax(tin, t1); tout = fmin(tout, t2);
+            }
+            if (miss || !(tout > tin)) continue;
+            const long long ka = (long long)ceil((tin - g.tau0) / g.step), ke = (long long)floor((tout - g.tau0) / g.step);
+            const int klo = (int)max(ka, 0LL), khi = (int)min(ke, (long long)g.K - 1);
+            for (int k = klo + lane; k <= khi; k += 32) {
+                // tau exactly as the scatter kernel forms it for a chunk starting at k: base in fp64, rounded once
+                const float tau = (float)(g.tau0 + (double)k * g.step);
+                const float X = fmaf(r.bx, tau, r.cx), Y = fmaf(r.by, tau, r.cy), Z = fmaf(r.bz, tau, r.cz);
+                const float fxf = floorf(X), fyf = floorf(Y), fzf = floorf(Z);
+                const int ix = (int)fxf, iy = (int)fyf, iz = (int)fzf;
+                const float wx = X - fxf, wy = Y - fyf, wz = Z - fzf;
+#pragma unroll
+                for (int cc = 0; cc < 8; ++cc) {
+                    const int x = ix + (cc & 1), y = iy + ((cc >> 1) & 1), z = iz + (cc >> 2);
+                    if ((unsigned)x >= (unsigned)g.nx || (unsigned)y >= (unsigned)g.ny || (unsigned)z >= (unsigned)g.nz) continue;
+                    const float w = ((cc & 1) ? wx : 1.f - wx) * ((cc & 2) ? wy : 1.f - wy) * ((cc & 4) ? wz : 1.f - wz);
+                    atomicAdd(acc_x + ((size_t)(z + pz) * (g.ny + ps) + (y + ps)) * (g.nx + pf) + (x + pf), round_mul(gq, w) * (1 << m));
+                }
+            }
+        }
+    }
+}
+
+// vol[z][y][x] (+)= (acc_x[z][y][x] + acc_y[z][x][y]) * step * T / 2^qb; 32x32 tiles, the y-fastest accumulator is
 // transposed through shared memory so that every global access is a coalesced row
 // (both accumulators carry a low-side margin of one box: pf x ps x pz elements, fast axis first)
 __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y,
@@ -309,7 +391,7 @@ __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__
     const size_t base_x = ((size_t)(blockIdx.z + pz) * (ny + ps) + ps) * (nx + pf) + pf;     // acc_x[z+pz][ps][pf]
     const size_t base_y = ((size_t)(blockIdx.z + pz) * (nx + ps) + ps) * (ny + pf) + pf;     // acc_y[z+pz][ps][pf]
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
-    const float k = __uint_as_float(__ldg(absmax_bits)) * step_over_two_qb;
+    const float k = __uint_as_float(__ldg(absmax_bits)) * step_over_two_qb;         // the fixed-point reference of the caller
     for (int j = threadIdx.y; j < 32; j += 8) {
         const int y = y0 + threadIdx.x, x = x0 + j;
         if (x < nx && y < ny) tile[j][threadIdx.x] = __ldg(acc_y + base_y + (size_t)x * (ny + pf) + y);
@@ -385,13 +467,15 @@ bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int
 void free_backproject_tma(cbct_geometry *G) {
     cudaFree(G->d_bt_acc);
     cudaFree(G->d_bt_absmax);
-    G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr; G->bt_ok = 0;
+    cudaFree(G->d_bt_sumsq); cudaFree(G->d_bt_partials); cudaFree(G->d_bt_counter);
+    G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr; G->d_bt_sumsq = G->d_bt_partials = nullptr; G->d_bt_counter = nullptr; G->bt_ok = 0;
 }
 
 // decide whether the scatter path runs for this geometry; needs the forward TMA box plan (same boxes)
 void plan_backproject_tma(cbct_geometry *G) {
     const cbct_geometry_desc &d = G->desc;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
+    G->d_bt_sumsq = G->d_bt_partials = nullptr; G->d_bt_counter = nullptr;
     if (!G->fw_tma_ok) return;
     // lane layout G->bt_lm (see the kernel; chosen by cbct_geometry_create): 0 = the skewed 8x4 layout, whose box is the
     // forward kernel's with the row count rounded up to a multiple of 4 (plane pitch = 0 mod 32); 1 = 16x2, forward's box
@@ -406,7 +490,9 @@ void plan_backproject_tma(cbct_geometry *G) {
     G->bt_acc_y_off = (n_acc + 31) & ~(size_t)31;
     G->bt_acc_elems = G->bt_acc_y_off + n_acc_y;
     if (cudaMalloc(&G->d_bt_acc, sizeof(int) * G->bt_acc_elems) != cudaSuccess ||
-        cudaMalloc(&G->d_bt_absmax, sizeof(unsigned)) != cudaSuccess) {
+        cudaMalloc(&G->d_bt_absmax, 2 * sizeof(unsigned)) != cudaSuccess || cudaMalloc(&G->d_bt_sumsq, sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&G->d_bt_partials, sizeof(double) * kReduceBlocks) != cudaSuccess ||
+        cudaMalloc(&G->d_bt_counter, sizeof(unsigned)) != cudaSuccess || cudaMemset(G->d_bt_counter, 0, sizeof(unsigned)) != cudaSuccess) {
         (void)cudaGetLastError();
         free_backproject_tma(G);
         return;
@@ -442,8 +528,11 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
     std::memcpy(&my, G->bt_map_y, sizeof(my));
     ScatterKernel kern = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, G->bt_packed != 0);
     if (!kern) return CBCT_E_UNSUPPORTED;
-    CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_absmax, 0, sizeof(unsigned), st));
+    CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_absmax, 0, 2 * sizeof(unsigned), st));
     absmax_kernel<<<592, 256, 0, st>>>(d_proj, (long long)G->n_rays, G->d_bt_absmax);
+    CBCT_LAUNCH_CHECK();
+    CBCT_TRY(launch_sumsq(d_proj, G->n_rays, G->d_bt_sumsq, G->d_bt_partials, G->d_bt_counter, st));
+    bt_reference_kernel<<<1, 1, 0, st>>>(G->d_bt_absmax, G->d_bt_sumsq, (double)G->n_rays);       // T = min(max|g|, 8 rms(g))
     CBCT_LAUNCH_CHECK();
     const size_t smem = bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz);
     // CBCT_FAULT: 0 outside the host-side test build; there, 8 = ignore the head-room plan (all views in one group)
@@ -453,11 +542,13 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
         const int nv_ = std::min(group, g.n_views - v0);
         CBCT_CUDA_TRY(cudaMemsetAsync(G->d_bt_acc, 0, sizeof(int) * G->bt_acc_elems, st));
         dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), nv_);
-        kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_proj, G->d_bt_acc, G->d_bt_absmax, two_qb, v0, G->fw_margin, G->bt_bz, G->err);
+        kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_proj, G->d_bt_acc, G->d_bt_absmax + 1, two_qb, v0, G->fw_margin, G->bt_bz, G->err);
+        CBCT_LAUNCH_CHECK();
+        backproject_outlier_kernel<<<296, 256, 0, st>>>(g, d_proj, G->d_bt_acc, G->d_bt_absmax + 1, two_qb, v0, nv_, G->bt_b, G->bt_bs, G->bt_bz);
         CBCT_LAUNCH_CHECK();
         dim3 fb(32, 8), fg(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
         backproject_finalize_kernel<<<fg, fb, 0, st>>>(G->d_bt_acc, G->d_bt_acc + G->bt_acc_y_off, d_vol, g.nx, g.ny, G->bt_b, G->bt_bs,
-                                                       G->bt_bz, G->d_bt_absmax,
+                                                       G->bt_bz, G->d_bt_absmax + 1,
                                                        (float)(G->step / std::ldexp(1.0, qb)), v0 > 0 ? 1 : 0, 1LL << 30, G->err);
         CBCT_LAUNCH_CHECK();
     }

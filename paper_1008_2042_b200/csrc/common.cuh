@@ -148,7 +148,9 @@ struct cbct_geometry {
     int bt_ok, bt_qb, bt_group;             // 2^bt_qb = fixed-point unit per max|g|; views per accumulation group
     int *d_bt_acc;
     size_t bt_acc_y_off, bt_acc_elems;      // element offset of the y-fastest accumulator, total elements
-    unsigned *d_bt_absmax;
+    unsigned *d_bt_absmax;                  // [0] bits of max|g|, [1] bits of the fixed-point reference T = min(max|g|, 8 rms(g))
+    double *d_bt_sumsq, *d_bt_partials;     // ||g||^2 (deterministic two-level reduction) and its scratch
+    unsigned *d_bt_counter;
     alignas(64) unsigned char bt_map_x[128];
     alignas(64) unsigned char bt_map_y[128];
     // Siddon pair (siddon.cu), allocated by cbct_siddon_prepare: y-fastest volume copy, two int32 accumulator volumes, max|g|

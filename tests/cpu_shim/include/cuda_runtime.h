@@ -125,6 +125,7 @@ static inline int __reduce_max_sync(unsigned m, int v) { return (int)shim::warp_
 static inline unsigned __reduce_max_sync(unsigned m, unsigned v) { return (unsigned)shim::warp_collective(m, shim::W_MAX_U32, v, 0); }
 static inline unsigned __reduce_min_sync(unsigned m, unsigned v) { return (unsigned)shim::warp_collective(m, shim::W_MIN_U32, v, 0); }
 static inline int __reduce_add_sync(unsigned m, int v) { return (int)shim::warp_collective(m, shim::W_ADD_S32, (uint64_t)(int64_t)v, 0); }
+static inline int __ffs(int v) { return __builtin_ffs(v); }
 static inline unsigned __ballot_sync(unsigned m, int pred) { return (unsigned)shim::warp_collective(m, shim::W_BALLOT, pred ? 1 : 0, 0); }
 template <class T>
 static inline T shim_shfl(unsigned m, shim::WarpOp op, T v, int arg) {

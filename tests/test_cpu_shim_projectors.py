@@ -173,6 +173,39 @@ def test_backproject_scatter_fixed_point_properties():
     assert rel_l2(f, op.back_scatter(G, ones.astype(np.float64))) <= TOL and np.all(f >= 0.0)
 
 
+def heavy_tailed_projections(G, seed):
+    """white noise (the hardest input for a fixed-point P^T: the result is small by cancellation) with a heavy tail:
+    a few dozen rays 20 .. 300 times the rms, both signs -- the shape of a CGLS residual of low-count Poisson data"""
+    rng = np.random.default_rng(seed)
+    y = rng.standard_normal(G.proj_shape).astype(np.float32) * 0.05
+    idx = rng.choice(y.size, 40, replace=False)
+    y.ravel()[idx] = (rng.choice([-1.0, 1.0], 40) * 0.05 * np.geomspace(20.0, 300.0, 40)).astype(np.float32)
+    return y
+
+
+@pytest.mark.parametrize("lanes,packed", [("1", "0"), ("0", "1")])
+def test_backproject_scatter_heavy_tailed_input(monkeypatch, lanes, packed):
+    """The fixed-point unit follows T = min(max|g|, 8 rms(g)), not the single largest value: rays above T are added by
+    backproject_outlier_kernel with their own unit.  Against the oracle at the usual bar (a unit tied to max|g|, 300 rms
+    here, would be 37 times coarser for every ray)."""
+    monkeypatch.setenv("CBCT_BT_LANES", lanes)
+    monkeypatch.setenv("CBCT_BT_PACKED", packed)
+    for G, seed in ((syn.workload(1).geometry, 37), (RAGGED_TMA, 38)):
+        y = heavy_tailed_projections(G, seed)
+        f = back(G, y)
+        log = sl.kernel_log()
+        assert "cbct::backproject_outlier_kernel" in log and any(k.startswith("cbct::backproject_scatter_kernel<") for k in log)
+        assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, (lanes, packed, G.nx)
+        assert np.array_equal(f, back(G, y))                                  # still integer sums: reproducible
+    # non-finite input is not laundered into finite numbers: the volume is NaN
+    G = syn.workload(1).geometry
+    y = syn.uniform_projections(G, 39)
+    y[2, 5, 7] = np.nan
+    assert np.all(np.isnan(back(G, y)))
+    y[2, 5, 7] = np.inf
+    assert np.all(np.isnan(back(G, y)))
+
+
 def test_degenerate_inputs():
     G = syn.workload(1).geometry
     assert np.all(forward(G, np.zeros(G.vol_shape, np.float32)) == 0.0)

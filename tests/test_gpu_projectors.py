@@ -196,12 +196,23 @@ def test_full_size_sampled_outputs(cfg):
     assert np.linalg.norm(got - ref) <= TOL * np.linalg.norm(ref)
     assert np.max(np.abs(got - ref)) <= 2e-5 * np.max(np.abs(ref))
     y = syn.uniform_projections(G, cfg)
-    f, _ = gpu_back(G, y)
+    f, hb = gpu_back(G, y)
     vox = np.sort(rng.choice(h.n_vox, 300, replace=False))
     vox[:4] = [0, G.nx - 1, h.n_vox - G.nx, h.n_vox - 1]                 # the four extreme corners too
     refv = op.back_gather_voxels(G, y.astype(np.float64), vox)
     gotv = f.ravel()[vox].astype(np.float64)
     assert np.linalg.norm(gotv - refv) <= TOL * np.linalg.norm(refv)
+    assert np.max(np.abs(gotv - refv)) <= 2e-5 * np.max(np.abs(refv))                 # per voxel, as for the rays above
+    # no guard of the TMA kernels was triggered (bounded waits, box range checks, fixed-point head-room)
+    assert h.status() == (True, []) and hb.status() == (True, [])
+    # the input that loads the int32 accumulators most: all ones (P^T of it IS the weight sum the head-room plan bounds)
+    ones = np.ones(G.proj_shape, np.float32)
+    f1, h1 = gpu_back(G, ones)
+    assert h1.status() == (True, []), "fixed-point head-room exhausted"
+    sub = vox[::6]
+    ref1 = op.back_gather_voxels(G, ones.astype(np.float64), sub)
+    assert np.linalg.norm(f1.ravel()[sub] - ref1) <= TOL * np.linalg.norm(ref1)
+    assert np.all(f1 >= 0.0)
     # property that holds at any size: adjoint identity
     x = syn.uniform_volume(G, cfg)
     Px, _ = gpu_forward(G, x)
@@ -258,6 +269,46 @@ def test_backproject_scatter_is_deterministic_and_scale_invariant():
     assert rel_l2(f, op.back_scatter(G, y_hot.astype(np.float64))) <= TOL
 
 
+def test_backproject_scatter_heavy_tailed_input_and_non_finite_input():
+    """White noise with a heavy tail (40 rays at 20 .. 300 rms, both signs: the shape of a CGLS residual of low-count
+    Poisson data).  The fixed-point unit follows T = min(max|g|, 8 rms(g)); rays above T are added by
+    backproject_outlier_kernel with their own unit, so the usual bar holds.  Non-finite input gives a NaN volume."""
+    for cfg in (1, 2):
+        G = syn.workload(cfg).geometry
+        rng = np.random.default_rng(37 + cfg)
+        y = rng.standard_normal(G.proj_shape).astype(np.float32) * 0.05
+        idx = rng.choice(y.size, 40, replace=False)
+        y.ravel()[idx] = (rng.choice([-1.0, 1.0], 40) * 0.05 * np.geomspace(20.0, 300.0, 40)).astype(np.float32)
+        f, h = gpu_back(G, y)
+        assert h.status() == (True, [])
+        assert rel_l2(f, op.back_scatter(G, y.astype(np.float64))) <= TOL, cfg
+        f2, _ = gpu_back(G, y)
+        assert np.array_equal(f, f2)
+    G = syn.workload(1).geometry
+    y = syn.uniform_projections(G, 39)
+    for bad in (np.nan, np.inf):
+        y[2, 5, 7] = bad
+        f, _ = gpu_back(G, y)
+        assert np.all(np.isnan(f))
+
+
+def test_poisson_residual_backprojection_at_paper_size():
+    """The input P^T actually sees inside CGLS at the paper-size config: the residual g - P f of Poisson data (5e4 photons
+    per ray, max(I,1) floor) against the noiseless phantom -- noise with a heavy tail where the body is thick.  Oracle on
+    sampled voxels (gather form), L2 and per-voxel bounds."""
+    w, ells, f0, g = syn.make_inputs(4)
+    G = w.geometry
+    r = g - syn.analytic_projections(G, ells)
+    f, h = gpu_back(G, r)
+    assert h.status() == (True, [])
+    rng = np.random.default_rng(4)
+    vox = np.sort(rng.choice(h.n_vox, 300, replace=False))
+    ref = op.back_gather_voxels(G, r.astype(np.float64), vox)
+    got = f.ravel()[vox].astype(np.float64)
+    assert np.linalg.norm(got - ref) <= TOL * np.linalg.norm(ref)
+    assert np.max(np.abs(got - ref)) <= 5e-5 * np.max(np.abs(ref))
+
+
 def test_backproject_scatter_headroom_bound():
     """The fixed-point plan assumes a bound on the sum of trilinear weights one voxel can receive; P^T of the
     all-ones projections IS that sum (times step), so it must stay below the planned head-room, and
@@ -269,6 +320,7 @@ def test_backproject_scatter_headroom_bound():
         ref = op.back_scatter(G, ones.astype(np.float64))
         assert rel_l2(f, ref) <= TOL
         assert np.all(f >= 0.0)
+        assert h.status() == (True, [])                                  # in particular: CBCT_STATUS_FIXED_POINT_RANGE not raised
 
 
 def test_backproject_gather_kernel_cross_check(monkeypatch):
