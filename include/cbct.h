@@ -237,6 +237,13 @@ int cbct_a2_extrapolate(const float *d_f_cur, const float *d_f_prev, float *d_v,
 typedef struct cbct_recon cbct_recon; /* opaque; owns per-level geometry, CGLS state and volumes */
 /* Allocates everything the cascade needs (finest nx, ny must be divisible by 2^(n_levels-1)). */
 int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels, cbct_recon **out);
+/* Same with options.  CBCT_RECON_BIN_DETECTOR: the level whose voxels are coarsened by a
+ * factor c in x,y works on projections binned by c (every c x c block of pixels replaced by its mean, pixel pitch
+ * x c, same detector centre; nu, nv must be divisible by 2^(n_levels-1)) -- the paper coarsens only the volume
+ * (PAPER.md:232 is silent on the data; reading of SURVEY.md §8(c) item 21), binning divides the rays of a coarse
+ * level by c^2.  The finest level always uses the full-resolution data. */
+enum { CBCT_RECON_BIN_DETECTOR = 1 };
+int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_levels, unsigned flags, cbct_recon **out);
 int cbct_recon_destroy(cbct_recon *recon);
 /* Runs the cascade asynchronously on `stream` (no allocation, no host synchronisation). */
 int cbct_recon_run(cbct_recon *recon, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu,

@@ -225,17 +225,30 @@ def a2(P, PT, g, f_init, n_outer, n_cgls, mu, momentum=True, trace=None):
     return f_cur
 
 
-def multigrid_a2(make_ops, finest_shape, g, n_levels, n_outer, n_cgls, mu, momentum=True):
+def bin_projections(g, factor):
+    """Detector binning: every factor x factor block of pixels of each view is replaced by
+    its mean, i.e. the line integral averaged over the block; `factor` a power of two.  g[view][v][u]."""
+    out = np.asarray(g, dtype=np.float64)
+    while factor > 1:
+        assert factor % 2 == 0
+        out = mg_restrict(out, 2, 2, 1)          # the "volume" axes (z, y, x) are (view, v, u) here: views are kept
+        factor //= 2
+    return out
+
+
+def multigrid_a2(make_ops, finest_shape, g, n_levels, n_outer, n_cgls, mu, momentum=True, bin_detector=False):
     """Coarse-to-fine cascade Omega_{2^(L-1) h} -> ... -> Omega_h: x,y coarsened by 2 per
-    level, z kept (item 20); g at full resolution on every level (item 21); the prolonged solution is
-    the initial guess and t, f^(k-1) are reset on each level (item 23).
+    level, z kept (item 20); g at full resolution on every level (item 21) unless bin_detector (NEXT-4: the level
+    coarsened by `fac` then works on g binned by `fac`, and make_ops must return the operators of the binned
+    detector); the prolonged solution is the initial guess and t, f^(k-1) are reset on each level (item 23).
     make_ops(level_factor) -> (P, PT) for the grid coarsened by `level_factor` in x and y."""
     nz, ny, nx = finest_shape
     fac = 2 ** (n_levels - 1)
     f = np.zeros((nz, ny // fac, nx // fac), dtype=np.float64)
     for lev in range(n_levels):
         P, PT = make_ops(fac)
-        f = a2(P, PT, g, f, n_outer[lev], n_cgls, mu, momentum)
+        g_lev = bin_projections(g, fac) if bin_detector else g
+        f = a2(P, PT, g_lev, f, n_outer[lev], n_cgls, mu, momentum)
         if lev + 1 < n_levels:
             f = mg_prolong(f, 2, 2, 1)
             fac //= 2

@@ -29,7 +29,7 @@ EXPORTS = [
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
-    "cbct_recon_create", "cbct_recon_destroy", "cbct_recon_run", "cbct_recon_run_host", "cbct_recon_status", "cbct_recon_describe",
+    "cbct_recon_create", "cbct_recon_create_ex", "cbct_recon_destroy", "cbct_recon_run", "cbct_recon_run_host", "cbct_recon_status", "cbct_recon_describe",
     "cbct_tf_reconstruct", "cbct_tf_reconstruct_host",
 ]
 
@@ -108,6 +108,7 @@ def _declare(L):
     L.mg_prolong.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
     L.cbct_a2_extrapolate.argtypes = [fp, fp, fp, C.c_float, C.c_int64, vp]
     L.cbct_recon_create.argtypes = [C.POINTER(GeometryDesc), ip, C.POINTER(vp)]
+    L.cbct_recon_create_ex.argtypes = [C.POINTER(GeometryDesc), ip, C.c_uint, C.POINTER(vp)]
     L.cbct_recon_destroy.argtypes = [vp]
     L.cbct_recon_run.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
     L.cbct_recon_run_host.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
@@ -408,10 +409,10 @@ def a2_extrapolate(d_f_cur, d_f_prev, d_v, coef: float, stream=None):
 class Recon:
     """cbct_recon handle: A2 inside the multigrid cascade."""
 
-    def __init__(self, geom, n_levels: int):
+    def __init__(self, geom, n_levels: int, bin_detector: bool = False):
         d, keep = make_desc(geom)
         h = C.c_void_p()
-        _check(lib().cbct_recon_create(C.byref(d), int(n_levels), C.byref(h)), "cbct_recon_create")
+        _check(lib().cbct_recon_create_ex(C.byref(d), int(n_levels), 1 if bin_detector else 0, C.byref(h)), "cbct_recon_create_ex")
         self.handle, self.n_levels, self.spec = h, int(n_levels), geom
         self.n_vox = geom.nx * geom.ny * geom.nz
         self.n_rays = len(tuple(geom.angles)) * geom.nv * geom.nu

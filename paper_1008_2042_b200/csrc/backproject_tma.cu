@@ -419,6 +419,7 @@ typedef void (*ScatterKernel)(DevGeom, const CUtensorMap, const CUtensorMap, con
                               float, int, DevErr);
 // two accumulator boxes (each a multiple of 128 bytes) + 128 bytes for the in-kernel alignment of the base
 static size_t bt_smem_bytes(int bf, int bs, int bz) { return (size_t)2 * ((bf * bs * bz + 31) & ~31) * 4 + 128; }
+constexpr size_t BT_SMEM_MAX = 101 * 1024;
 static ScatterKernel scatter_kernel_ptr(int bf, int bs, int lm, bool pk) {
 #define CBCT_SK(F, S, L) \
     if (bf == F && bs == S && lm == L) return pk ? backproject_scatter_kernel<F, S, L, true> : backproject_scatter_kernel<F, S, L, false>;
@@ -480,7 +481,7 @@ void plan_backproject_tma(cbct_geometry *G) {
     // lane layout G->bt_lm (see the kernel; chosen by cbct_geometry_create): 0 = the skewed 8x4 layout, whose box is the
     // forward kernel's with the row count rounded up to a multiple of 4 (plane pitch = 0 mod 32); 1 = 16x2, forward's box
     G->bt_b = G->fw_b; G->bt_bz = G->fw_bz; G->bt_bs = G->bt_lm == 0 ? (G->fw_bs + 3) & ~3 : G->fw_bs;
-    if (bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz) > 101 * 1024) return;
+    if (bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz) > BT_SMEM_MAX) return;
     int qb = 0, group = 0;
     double w_view = 0;
     if (!bt_fixed_point_plan(d, G->R, G->step, &qb, &group, &w_view)) return;
@@ -510,8 +511,9 @@ void plan_backproject_tma(cbct_geometry *G) {
     std::memcpy(G->bt_map_y, &my, sizeof(my));
     for (int pk = 0; pk < 2; ++pk) {
         ScatterKernel k = scatter_kernel_ptr(G->bt_b, G->bt_bs, G->bt_lm, pk != 0);
-        if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)bt_smem_bytes(G->bt_b, G->bt_bs, G->bt_bz)) != cudaSuccess) {
+        // the attribute belongs to the kernel, not to the handle: always the plan's limit, never this geometry's need
+        if (!k || cudaFuncSetAttribute(reinterpret_cast<const void *>(k), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BT_SMEM_MAX) !=
+                      cudaSuccess) {
             (void)cudaGetLastError();
             free_backproject_tma(G);
             return;

@@ -11,7 +11,8 @@ struct cbct_recon_level {
     cbct_geometry *geom;
     cbct_cgls *cg;
     float *d_x, *d_p, *d_fa, *d_fb, *d_fc;   // volume-sized: CGLS x, p; A2 f^(k), f^(k-1), scratch
-    int nx, ny, nz;
+    float *d_gbin;                            // this level's binned projections (CBCT_RECON_BIN_DETECTOR, coarse levels), else null
+    int nx, ny, nz, nu, nv;
 };
 
 struct cbct_recon {
@@ -29,7 +30,7 @@ extern "C" int cbct_recon_destroy(cbct_recon *R) {
     for (auto &L : R->lev) {
         cbct_cgls_destroy(L.cg);
         cbct_geometry_destroy(L.geom);
-        cudaFree(L.d_x); cudaFree(L.d_p); cudaFree(L.d_fa); cudaFree(L.d_fb); cudaFree(L.d_fc);
+        cudaFree(L.d_x); cudaFree(L.d_p); cudaFree(L.d_fa); cudaFree(L.d_fb); cudaFree(L.d_fc); cudaFree(L.d_gbin);
     }
     cudaFree(R->d_r); cudaFree(R->d_g); cudaFree(R->d_f);
     (void)cudaGetLastError();
@@ -38,10 +39,16 @@ extern "C" int cbct_recon_destroy(cbct_recon *R) {
 }
 
 extern "C" int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels, cbct_recon **out) {
-    if (!finest || !out || n_levels < 1 || n_levels > 8) return CBCT_E_INVALID;
+    return cbct_recon_create_ex(finest, n_levels, 0u, out);
+}
+
+extern "C" int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_levels, unsigned flags, cbct_recon **out) {
+    if (!finest || !out || n_levels < 1 || n_levels > 8 || (flags & ~(unsigned)CBCT_RECON_BIN_DETECTOR)) return CBCT_E_INVALID;
     *out = nullptr;
     const int fac0 = 1 << (n_levels - 1);
     if (finest->nx % fac0 || finest->ny % fac0) return CBCT_E_INVALID;   // x,y coarsened by 2 per level, z kept
+    const bool bin = (flags & CBCT_RECON_BIN_DETECTOR) != 0;
+    if (bin && (finest->nu % fac0 || finest->nv % fac0)) return CBCT_E_INVALID;
     cbct_recon *R = new (std::nothrow) cbct_recon();
     if (!R) return CBCT_E_INVALID;
     R->n_levels = n_levels;
@@ -54,8 +61,16 @@ extern "C" int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels,
         cbct_geometry_desc d = *finest;
         d.nx = finest->nx / fac; d.ny = finest->ny / fac;
         d.dx = finest->dx * fac; d.dy = finest->dy * fac;             // same extent, coarser pitch
+        if (bin) {                                                    // NEXT-4: same detector extent and centre, coarser pixels
+            d.nu = finest->nu / fac; d.nv = finest->nv / fac;
+            d.du = finest->du * fac; d.dv = finest->dv * fac;
+        }
         cbct_recon_level L{};
-        L.nx = d.nx; L.ny = d.ny; L.nz = d.nz;
+        L.nx = d.nx; L.ny = d.ny; L.nz = d.nz; L.nu = d.nu; L.nv = d.nv;
+        if (bin && fac > 1) {
+            cudaError_t e = cudaMalloc(&L.d_gbin, sizeof(float) * (size_t)d.nu * d.nv * d.n_views);
+            if (e != cudaSuccess) status = set_cuda_error(e);
+        }
         status = cbct_geometry_create(&d, &L.geom);
         if (status == CBCT_OK) status = cbct_cgls_create(L.geom, &L.cg);
         const size_t bytes = sizeof(float) * (size_t)d.nx * d.ny * d.nz;
@@ -83,8 +98,16 @@ extern "C" int cbct_recon_run(cbct_recon *R, const float *d_g, float *d_f, const
                               int momentum, void *stream) {
     if (!R || !d_g || !d_f || !n_outer || n_cgls < 0 || !(mu >= 0.f)) return CBCT_E_INVALID;
     cudaStream_t st = as_stream(stream);
+    // detector binning: level l's data = block means of level l+1's (finest = d_g), i.e. mg_restrict on [view][v][u]
+    for (int l = R->n_levels - 2; l >= 0; --l) {
+        cbct_recon_level &L = R->lev[l], &F = R->lev[l + 1];
+        if (!L.d_gbin) continue;
+        const int n_views = (int)(R->n_rays / ((int64_t)R->lev.back().nu * R->lev.back().nv));
+        CBCT_TRY(mg_restrict(F.d_gbin ? F.d_gbin : d_g, L.d_gbin, F.nu, F.nv, n_views, 2, 2, 1, stream));
+    }
     for (int l = 0; l < R->n_levels; ++l) {
         cbct_recon_level &L = R->lev[l];
+        const float *g_l = L.d_gbin ? L.d_gbin : d_g;
         const int64_t n = (int64_t)L.nx * L.ny * L.nz;
         float *f_cur = L.d_fa, *f_prev = L.d_fb, *f_new = L.d_fc;
         if (l == 0) {
@@ -98,7 +121,7 @@ extern "C" int cbct_recon_run(cbct_recon *R, const float *d_g, float *d_f, const
         for (int k = 0; k < n_outer[l]; ++k) {
             const float coef = momentum ? (float)((t_prev - 1.0) / t_cur) : 0.f;
             CBCT_TRY(cbct_a2_extrapolate(f_cur, f_prev, L.d_x, coef, n, stream));        // 1. v
-            CBCT_TRY(cbct_cgls_init(L.cg, d_g, L.d_x, R->d_r, L.d_p, stream));           // 2. f = CGLS[v]
+            CBCT_TRY(cbct_cgls_init(L.cg, g_l, L.d_x, R->d_r, L.d_p, stream));           // 2. f = CGLS[v]
             for (int m = 0; m < n_cgls; ++m) CBCT_TRY(cbct_cgls_step(L.cg, L.d_x, R->d_r, L.d_p, stream));
             CBCT_TRY(tf_apply_fused(L.d_x, f_new, mu, 1, L.nx, L.ny, L.nz, stream));     // 3.+4. shrink, clamp
             float *tmp = f_prev; f_prev = f_cur; f_cur = f_new; f_new = tmp;

@@ -300,6 +300,7 @@ static TmaKernel tma_kernel_ptr(int bf, int bs, bool pk) {
 
 // two boxes (each a multiple of 128 bytes) + 128 bytes for the in-kernel alignment of the base
 static size_t fw_tma_smem_bytes(int bf, int bs, int bz) { return (size_t)2 * ((bf * bs * bz + 31) & ~31) * 4 + 128; }
+constexpr size_t FW_TMA_SMEM_MAX = 97 * 1024;        // two boxes of <= 48 KiB: two CTAs per SM
 
 // choose the box for this geometry (once, at create); fw_tma_ok = 0 when the TMA path cannot be used
 void plan_forward_tma(cbct_geometry *G) {
@@ -327,7 +328,7 @@ void plan_forward_tma(cbct_geometry *G) {
     for (auto &m : menu)
         if (m[0] >= need_f && m[1] >= need_s) { bf = m[0]; bs = m[1]; break; }
     if (!bf || bz > 32) return;
-    if ((size_t)2 * bf * bs * bz * 4 > 96 * 1024) return;
+    if (fw_tma_smem_bytes(bf, bs, bz) > FW_TMA_SMEM_MAX) return;
     G->fw_b = bf; G->fw_bs = bs; G->fw_bz = bz; G->fw_margin = (float)margin;
     if (cudaMalloc(&G->d_fw_volT, sizeof(float) * G->n_vox) != cudaSuccess) { (void)cudaGetLastError(); G->d_fw_volT = nullptr; return; }
     G->workspace_bytes += sizeof(float) * G->n_vox;
@@ -337,7 +338,8 @@ void plan_forward_tma(cbct_geometry *G) {
     std::memcpy(G->fw_map_y, &m, sizeof(m));
     for (int pk = 0; pk < 2; ++pk) {
         const void *kern = reinterpret_cast<const void *>(tma_kernel_ptr(bf, bs, pk != 0));
-        if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fw_tma_smem_bytes(bf, bs, bz)) != cudaSuccess) {
+        // the attribute belongs to the kernel, not to the handle: always the plan's limit, never this geometry's need
+        if (!kern || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FW_TMA_SMEM_MAX) != cudaSuccess) {
             (void)cudaGetLastError();
             return;
         }

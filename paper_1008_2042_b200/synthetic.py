@@ -81,6 +81,20 @@ class Geometry:
                        dx=self.dx * factor, dy=self.dy * factor)
 
 
+    def bin_detector(self, factor: int = 2) -> "Geometry":
+        """Same detector extent and centre, pixel pitch x`factor` (detector binning at the
+        coarse multigrid levels; block (i, j) of factor x factor pixels becomes one pixel at the block's centre)."""
+        assert self.nu % factor == 0 and self.nv % factor == 0
+        return replace(self, nu=self.nu // factor, nv=self.nv // factor, du=self.du * factor, dv=self.dv * factor)
+
+
+def short_scan(n_views: int, arc_deg: float = 200.0, start_deg: float = -10.0) -> Tuple[float, ...]:
+    """n views evenly over an arc, BOTH endpoints included (the scanner's "200 deg ... arcs"; SURVEY.md
+    §8(f) NEXT-4).  The default arc, -10 deg .. 190 deg, is 180 deg + a 20 deg fan margin."""
+    a0, arc = math.radians(start_deg), math.radians(arc_deg)
+    return tuple(a0 + arc * k / (n_views - 1) for k in range(n_views))
+
+
 def full_circle(n_views: int) -> Tuple[float, ...]:
     """theta_k = 2 pi k / n, endpoint excluded."""
     return tuple(2.0 * math.pi * k / n_views for k in range(n_views))

@@ -246,3 +246,19 @@ def tf_reconstruct_volume(geom, g, n_levels, n_outer, n_cgls=3, mu=5e-4, momentu
     check(lib().cbct_tf_reconstruct(C.byref(d), g.ptr, out.ptr, int(n_levels), arr, int(n_cgls), float(mu), int(bool(momentum)), None),
           "cbct_tf_reconstruct")
     return out
+
+
+def recon_run(geom, g, n_levels, n_outer, n_cgls=3, mu=5e-4, momentum=True, bin_detector=False):
+    """cbct_recon_create_ex + cbct_recon_run + cbct_recon_status + destroy"""
+    d, keep = cb.make_desc(geom)
+    h = C.c_void_p()
+    check(lib().cbct_recon_create_ex(C.byref(d), int(n_levels), 1 if bin_detector else 0, C.byref(h)), "cbct_recon_create_ex")
+    arr = (C.c_int * n_levels)(*[int(v) for v in n_outer])
+    out = Buf((geom.nz, geom.ny, geom.nx))
+    try:
+        check(lib().cbct_recon_run(h, g.ptr, out.ptr, arr, int(n_cgls), float(mu), int(bool(momentum)), None), "cbct_recon_run")
+        flags = C.c_int(0)
+        check(lib().cbct_recon_status(h, None, C.byref(flags), 0), "cbct_recon_status")
+    finally:
+        lib().cbct_recon_destroy(h)
+    return out

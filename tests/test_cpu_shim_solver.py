@@ -127,6 +127,28 @@ def test_multigrid_a2_driver_two_levels():
     assert rel(out, ref) <= 1e-4
 
 
+def test_short_scan_cascade_with_detector_binning():
+    """a 200-degree arc (unequal orientation phases, endpoints included) through the
+    two-level driver, with and without detector binning at the coarse level, against the oracle's cascade."""
+    G = syn.Geometry(32, 32, 8, 4.0, 4.0, 4.0, 48, 16, 3.2, 3.2, 1000.0, 1500.0, syn.short_scan(11, 200.0, -10.0))
+    f0 = syn.uniform_volume(G, 82)
+    g = op.forward(G, f0.astype(np.float64)).astype(np.float32)
+    mu, n_outer, n_cgls = 5e-4, [2, 2], 2
+    for binned in (False, True):
+        def make_ops(fac, binned=binned):
+            Gl = G.coarsen_xy(fac) if fac > 1 else G
+            return ops(Gl.bin_detector(fac) if (binned and fac > 1) else Gl)
+        ref = osv.multigrid_a2(make_ops, G.vol_shape, g.astype(np.float64), 2, n_outer, n_cgls, mu, bin_detector=binned)
+        out = sl.recon_run(G, sl.dev(g), 2, n_outer, n_cgls, mu, True, bin_detector=binned).numpy()
+        assert rel(out, ref) <= 1e-4, binned
+    import ctypes as C
+    from paper_1008_2042_b200 import binding as cb
+    d, _keep = cb.make_desc(syn.Geometry(32, 32, 8, 4.0, 4.0, 4.0, 47, 16, 3.2, 3.2, 1000.0, 1500.0, (0.0, 1.0)))
+    h = C.c_void_p()
+    assert sl.lib().cbct_recon_create_ex(C.byref(d), 2, 1, C.byref(h)) == cb.CBCT_E_INVALID      # 47 pixels do not bin by 2
+    assert sl.lib().cbct_recon_create_ex(C.byref(d), 2, 6, C.byref(h)) == cb.CBCT_E_INVALID      # unknown flag
+
+
 def test_microbench_kernels_stay_in_bounds():
     """cbct_microbench (SURVEY.md §8(d) denominators) with its timed loops shortened: every kernel runs under the shim's
     guards and alignment checks; the rates themselves mean nothing on the host."""

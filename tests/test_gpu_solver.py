@@ -254,3 +254,32 @@ def test_multigrid_cascade_matches_oracle_two_levels():
     rrms = rel(host(d_f), f0.astype(np.float64))                # PAPER.md:270 RRMS (context, synthetic phantom)
     print("RRMS vs phantom after 3+3 outer iterations:", rrms)
     assert rrms < 0.5
+
+
+def test_short_scan_cascade_with_detector_binning():
+    """the scanner's 200-degree arc (20 views, endpoints included) on the config-2
+    volume and detector, two levels, with and without detector binning at the coarse level (cbct_recon_create_ex),
+    against the oracle's cascade; P and P^T of the arc geometry on their own first."""
+    w, ells, f0, _ = syn.make_inputs(2, noisy=False)
+    G = w.geometry.with_views(syn.short_scan(20, 200.0, -10.0))
+    g = syn.analytic_projections(G, ells)
+    h = cb.Geometry(G)
+    d_p = torch.empty(h.proj_shape, dtype=torch.float32, device="cuda")
+    d_v = torch.empty(h.vol_shape, dtype=torch.float32, device="cuda")
+    h.forward(dev(f0), d_p)
+    h.backproject(dev(g), d_v)
+    assert rel(host(d_p), op.forward(G, f0.astype(np.float64))) <= 1e-5
+    assert rel(host(d_v), op.back_scatter(G, g.astype(np.float64))) <= 1e-5
+    assert h.status() == (True, [])
+    mu, n_outer, n_cgls = 5e-4, [2, 2], 2
+    for binned in (False, True):
+        def make_ops(fac, binned=binned):
+            Gl = G.coarsen_xy(fac) if fac > 1 else G
+            return ops(Gl.bin_detector(fac) if (binned and fac > 1) else Gl)
+        ref = osv.multigrid_a2(make_ops, G.vol_shape, g.astype(np.float64), 2, n_outer, n_cgls, mu, bin_detector=binned)
+        rec = cb.Recon(G, 2, bin_detector=binned)
+        d_f = torch.empty(G.vol_shape, dtype=torch.float32, device="cuda")
+        rec.run(dev(g), d_f, n_outer, n_cgls, mu, True)
+        assert rec.status() == (True, [])
+        assert rel(host(d_f), ref) <= 1e-4, binned
+        rec.close()
