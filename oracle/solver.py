@@ -204,11 +204,13 @@ def a2_t_next(t):
     return 0.5 * (1.0 + math.sqrt(1.0 + 4.0 * t * t))
 
 
-def a2(P, PT, g, f_init, n_outer, n_cgls, mu, momentum=True, trace=None):
+def a2(P, PT, g, f_init, n_outer, n_cgls, mu, momentum=True, trace=None, regulariser=None):
     """Algorithm A2; momentum=False gives Algorithm A1.
     Step 1 is garbled in PAPER.md:165; reading of item 11:
         v = f^k + ((t^(k-1) - 1)/t^k) (f^k - f^(k-1)),  t^(-1) = t^(0) = 1, f^(-1) = f^(0) = f_init.
-    CGLS restarts from x0 = v every outer iteration (item 23)."""
+    CGLS restarts from x0 = v every outer iteration (item 23).
+    regulariser: a callable x -> x' that replaces the tight-frame shrinkage of step 3 (the TV comparison
+    algorithm is "akin to the Algorithm A1", with the ROF sub-problem in that place; oracle/tv.py); mu is then unused."""
     f_prev = np.array(f_init, dtype=np.float64, copy=True)
     f_cur = f_prev.copy()
     t_prev, t_cur = 1.0, 1.0
@@ -216,7 +218,7 @@ def a2(P, PT, g, f_init, n_outer, n_cgls, mu, momentum=True, trace=None):
         coef = (t_prev - 1.0) / t_cur if momentum else 0.0
         v = f_cur + coef * (f_cur - f_prev)                    # 1. extrapolate
         x, hist = cgls(P, PT, v, g, n_cgls)                     # 2. f = CGLS[v]
-        x = tf_apply(x, mu, clamp_nonneg=False)                 # 3. shrinkage
+        x = tf_apply(x, mu, clamp_nonneg=False) if regulariser is None else regulariser(x)   # 3. shrinkage (or ROF)
         x = positivity(x)                                       # 4. correct
         if trace is not None:
             trace.append(dict(k=k, coef=coef, t=t_cur, rr=hist))
@@ -236,7 +238,7 @@ def bin_projections(g, factor):
     return out
 
 
-def multigrid_a2(make_ops, finest_shape, g, n_levels, n_outer, n_cgls, mu, momentum=True, bin_detector=False):
+def multigrid_a2(make_ops, finest_shape, g, n_levels, n_outer, n_cgls, mu, momentum=True, bin_detector=False, regulariser=None):
     """Coarse-to-fine cascade Omega_{2^(L-1) h} -> ... -> Omega_h: x,y coarsened by 2 per
     level, z kept (item 20); g at full resolution on every level (item 21) unless bin_detector (NEXT-4: the level
     coarsened by `fac` then works on g binned by `fac`, and make_ops must return the operators of the binned
@@ -248,7 +250,7 @@ def multigrid_a2(make_ops, finest_shape, g, n_levels, n_outer, n_cgls, mu, momen
     for lev in range(n_levels):
         P, PT = make_ops(fac)
         g_lev = bin_projections(g, fac) if bin_detector else g
-        f = a2(P, PT, g_lev, f, n_outer[lev], n_cgls, mu, momentum)
+        f = a2(P, PT, g_lev, f, n_outer[lev], n_cgls, mu, momentum, regulariser=regulariser)
         if lev + 1 < n_levels:
             f = mg_prolong(f, 2, 2, 1)
             fac //= 2
