@@ -213,6 +213,23 @@ int tf_apply_fused(const float *d_in, float *d_out, float mu, int clamp_nonneg, 
                    void *stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * The paper's COMPARISON regulariser: total variation through the Rudin-Osher-Fatemi
+ * sub-problem:  f = argmin ||f - u||^2 + mu_tv ||f||_TV  "by a simple gradient descent method ...
+ * with an adaptively adjusted step length", stopped when the energy decreases by less than rel_tol (the paper: 0.1 %).
+ * Discretisation (the paper gives none; DESIGN.md §1b T1-T6): forward differences, zero across the last faces;
+ * isotropic TV smoothed as sqrt(|Df|^2 + eps^2), eps > 0 in the units of f; a trial step f - tau grad E is accepted
+ * iff it lowers E (tau *= 1.2, else tau /= 2; tau starts at 0.25, f at u); stop at the first accepted step with
+ * (E_k - E_k+1)/E_k < rel_tol, after max_iter trials, or at once if E(u) = 0.  The control state lives in device
+ * memory: asynchronous on `stream`, nothing is read back.  clamp_nonneg != 0 applies H = max(.,0) to the result.
+ * d_work: caller-owned device scratch of tv_rof_workspace_bytes(nx,ny,nz) bytes (256-byte aligned).  d_u != d_f.
+ * tv_rof_result synchronises `stream` and reports the trials used, the accepted steps and the final energy.
+ * ---------------------------------------------------------------------------------------------- */
+size_t tv_rof_workspace_bytes(int nx, int ny, int nz);
+int tv_rof(const float *d_u, float *d_f, void *d_work, float mu_tv, float eps, int max_iter, float rel_tol,
+           int clamp_nonneg, int nx, int ny, int nz, void *stream);
+int tv_rof_result(const void *d_work, int nx, int ny, int nz, int *trials, int *accepted, double *energy, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
  * Multigrid transfers (§2.2.3).  Per-axis factors fx,fy,fz in {1,2}; fine sizes must be
  * divisible.  restrict = mean of the children; prolong = cell-centred linear interpolation (weights
  * 3/4, 1/4, neighbour clamped at the faces).
@@ -242,12 +259,17 @@ int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels, cbct_recon
  * x c, same detector centre; nu, nv must be divisible by 2^(n_levels-1)) -- the paper coarsens only the volume
  * (PAPER.md:232 is silent on the data; reading of SURVEY.md §8(c) item 21), binning divides the rays of a coarse
  * level by c^2.  The finest level always uses the full-resolution data. */
-enum { CBCT_RECON_BIN_DETECTOR = 1 };
+enum { CBCT_RECON_BIN_DETECTOR = 1, CBCT_RECON_TV = 2 /* also allocate the workspace cbct_recon_run_tv needs */ };
 int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_levels, unsigned flags, cbct_recon **out);
 int cbct_recon_destroy(cbct_recon *recon);
 /* Runs the cascade asynchronously on `stream` (no allocation, no host synchronisation). */
 int cbct_recon_run(cbct_recon *recon, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu,
                    int momentum, void *stream);
+/* The TV comparison algorithm of PAPER.md:236 on the same cascade: as cbct_recon_run, with the tight-frame shrinkage of
+ * every outer iteration replaced by tv_rof(mu_tv, eps, max_rof_iter, rel_tol) followed by H.  The handle must have been
+ * created with CBCT_RECON_TV (CBCT_E_INVALID otherwise). */
+int cbct_recon_run_tv(cbct_recon *recon, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu_tv,
+                      float eps, int max_rof_iter, float rel_tol, int momentum, void *stream);
 /* HOST buffers: h_g -> device, run, volume -> h_f; synchronises `stream` before returning. */
 int cbct_recon_run_host(cbct_recon *recon, const float *h_g, float *h_f, const int *n_outer, int n_cgls,
                         float mu, int momentum, void *stream);

@@ -28,7 +28,7 @@ EXPORTS = [
     "cbct_siddon_fixed_point_plan", "cbct_microbench", "tf_reconstruct_direct",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
-    "mg_restrict", "mg_prolong", "cbct_a2_extrapolate",
+    "mg_restrict", "mg_prolong", "cbct_a2_extrapolate", "tv_rof_workspace_bytes", "tv_rof", "tv_rof_result", "cbct_recon_run_tv",
     "cbct_recon_create", "cbct_recon_create_ex", "cbct_recon_destroy", "cbct_recon_run", "cbct_recon_run_host", "cbct_recon_status", "cbct_recon_describe",
     "cbct_tf_reconstruct", "cbct_tf_reconstruct_host",
 ]
@@ -107,6 +107,10 @@ def _declare(L):
     L.mg_restrict.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
     L.mg_prolong.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
     L.cbct_a2_extrapolate.argtypes = [fp, fp, fp, C.c_float, C.c_int64, vp]
+    L.tv_rof_workspace_bytes.argtypes = [ip, ip, ip]
+    L.tv_rof.argtypes = [fp, fp, vp, C.c_float, C.c_float, ip, C.c_float, ip, ip, ip, ip, vp]
+    L.tv_rof_result.argtypes = [vp, ip, ip, ip, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_double), vp]
+    L.cbct_recon_run_tv.argtypes = [vp, fp, fp, C.POINTER(C.c_int), ip, C.c_float, C.c_float, ip, C.c_float, ip, vp]
     L.cbct_recon_create.argtypes = [C.POINTER(GeometryDesc), ip, C.POINTER(vp)]
     L.cbct_recon_create_ex.argtypes = [C.POINTER(GeometryDesc), ip, C.c_uint, C.POINTER(vp)]
     L.cbct_recon_destroy.argtypes = [vp]
@@ -120,6 +124,7 @@ def _declare(L):
         if name != "cbct_status_string":
             getattr(L, name).restype = C.c_int
     L.cbct_launch_count.restype = C.c_longlong
+    L.tv_rof_workspace_bytes.restype = C.c_size_t
     return L
 
 
@@ -385,6 +390,18 @@ def tf_apply_fused(d_in, d_out, mu: float, clamp_nonneg: bool = False, stream=No
     return d_out
 
 
+def tv_rof(d_u, d_f, mu_tv: float, eps: float, max_iter: int = 30, rel_tol: float = 1e-3, clamp_nonneg: bool = False, stream=None):
+    """PAPER.md:236 ROF sub-problem (tv_rof); returns (d_f, trials, accepted, energy) -- reading them back synchronises."""
+    import torch
+    nx, ny, nz = _dims(d_u.shape)
+    work = torch.empty(int(lib().tv_rof_workspace_bytes(nx, ny, nz)), dtype=torch.uint8, device=d_u.device)
+    _check(lib().tv_rof(_dptr(d_u), _dptr(d_f, nx * ny * nz), work.data_ptr(), float(mu_tv), float(eps), int(max_iter), float(rel_tol),
+                        int(bool(clamp_nonneg)), nx, ny, nz, _stream(stream)), "tv_rof")
+    tr, ac, en = C.c_int(), C.c_int(), C.c_double()
+    _check(lib().tv_rof_result(work.data_ptr(), nx, ny, nz, C.byref(tr), C.byref(ac), C.byref(en), _stream(stream)), "tv_rof_result")
+    return d_f, tr.value, ac.value, en.value
+
+
 def mg_restrict(d_fine, d_coarse, fx=2, fy=2, fz=1, stream=None):
     nx, ny, nz = _dims(d_fine.shape)
     _check(lib().mg_restrict(_dptr(d_fine), _dptr(d_coarse, (nx // fx) * (ny // fy) * (nz // fz)), nx, ny, nz, fx, fy, fz,
@@ -409,10 +426,11 @@ def a2_extrapolate(d_f_cur, d_f_prev, d_v, coef: float, stream=None):
 class Recon:
     """cbct_recon handle: A2 inside the multigrid cascade."""
 
-    def __init__(self, geom, n_levels: int, bin_detector: bool = False):
+    def __init__(self, geom, n_levels: int, bin_detector: bool = False, tv: bool = False):
         d, keep = make_desc(geom)
         h = C.c_void_p()
-        _check(lib().cbct_recon_create_ex(C.byref(d), int(n_levels), 1 if bin_detector else 0, C.byref(h)), "cbct_recon_create_ex")
+        _check(lib().cbct_recon_create_ex(C.byref(d), int(n_levels), (1 if bin_detector else 0) | (2 if tv else 0), C.byref(h)),
+               "cbct_recon_create_ex")
         self.handle, self.n_levels, self.spec = h, int(n_levels), geom
         self.n_vox = geom.nx * geom.ny * geom.nz
         self.n_rays = len(tuple(geom.angles)) * geom.nv * geom.nu
@@ -448,6 +466,13 @@ class Recon:
     def run(self, d_g, d_f, n_outer, n_cgls=3, mu=5e-4, momentum=True, stream=None):
         _check(lib().cbct_recon_run(self.handle, _dptr(d_g, self.n_rays), _dptr(d_f, self.n_vox), self._outer(n_outer),
                                     int(n_cgls), float(mu), int(bool(momentum)), _stream(stream)), "cbct_recon_run")
+        return d_f
+
+    def run_tv(self, d_g, d_f, n_outer, n_cgls=3, mu_tv=1e-3, eps=1e-4, max_rof_iter=30, rel_tol=1e-3, momentum=True, stream=None):
+        """the TV comparison algorithm on the same cascade; the handle needs tv=True"""
+        _check(lib().cbct_recon_run_tv(self.handle, _dptr(d_g, self.n_rays), _dptr(d_f, self.n_vox), self._outer(n_outer), int(n_cgls),
+                                       float(mu_tv), float(eps), int(max_rof_iter), float(rel_tol), int(bool(momentum)),
+                                       _stream(stream)), "cbct_recon_run_tv")
         return d_f
 
     def run_host(self, h_g, h_f, n_outer, n_cgls=3, mu=5e-4, momentum=True, stream=None):

@@ -12,6 +12,7 @@ struct cbct_recon_level {
     cbct_cgls *cg;
     float *d_x, *d_p, *d_fa, *d_fb, *d_fc;   // volume-sized: CGLS x, p; A2 f^(k), f^(k-1), scratch
     float *d_gbin;                            // this level's binned projections (CBCT_RECON_BIN_DETECTOR, coarse levels), else null
+    void *d_tv_work;                          // scratch of tv_rof (CBCT_RECON_TV), else null
     int nx, ny, nz, nu, nv;
 };
 
@@ -30,7 +31,7 @@ extern "C" int cbct_recon_destroy(cbct_recon *R) {
     for (auto &L : R->lev) {
         cbct_cgls_destroy(L.cg);
         cbct_geometry_destroy(L.geom);
-        cudaFree(L.d_x); cudaFree(L.d_p); cudaFree(L.d_fa); cudaFree(L.d_fb); cudaFree(L.d_fc); cudaFree(L.d_gbin);
+        cudaFree(L.d_x); cudaFree(L.d_p); cudaFree(L.d_fa); cudaFree(L.d_fb); cudaFree(L.d_fc); cudaFree(L.d_gbin); cudaFree(L.d_tv_work);
     }
     cudaFree(R->d_r); cudaFree(R->d_g); cudaFree(R->d_f);
     (void)cudaGetLastError();
@@ -43,7 +44,7 @@ extern "C" int cbct_recon_create(const cbct_geometry_desc *finest, int n_levels,
 }
 
 extern "C" int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_levels, unsigned flags, cbct_recon **out) {
-    if (!finest || !out || n_levels < 1 || n_levels > 8 || (flags & ~(unsigned)CBCT_RECON_BIN_DETECTOR)) return CBCT_E_INVALID;
+    if (!finest || !out || n_levels < 1 || n_levels > 8 || (flags & ~(unsigned)(CBCT_RECON_BIN_DETECTOR | CBCT_RECON_TV))) return CBCT_E_INVALID;
     *out = nullptr;
     const int fac0 = 1 << (n_levels - 1);
     if (finest->nx % fac0 || finest->ny % fac0) return CBCT_E_INVALID;   // x,y coarsened by 2 per level, z kept
@@ -71,6 +72,10 @@ extern "C" int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_leve
             cudaError_t e = cudaMalloc(&L.d_gbin, sizeof(float) * (size_t)d.nu * d.nv * d.n_views);
             if (e != cudaSuccess) status = set_cuda_error(e);
         }
+        if ((flags & CBCT_RECON_TV) && status == CBCT_OK) {
+            cudaError_t e = cudaMalloc(&L.d_tv_work, tv_rof_workspace_bytes(d.nx, d.ny, d.nz));
+            if (e != cudaSuccess) status = set_cuda_error(e);
+        }
         status = cbct_geometry_create(&d, &L.geom);
         if (status == CBCT_OK) status = cbct_cgls_create(L.geom, &L.cg);
         const size_t bytes = sizeof(float) * (size_t)d.nx * d.ny * d.nz;
@@ -94,9 +99,28 @@ extern "C" int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_leve
     return CBCT_OK;
 }
 
+// the regulariser of A2 steps 3-4: the tight frame or the TV comparison
+struct Regulariser { bool tv; float mu, eps, rel_tol; int max_iter; };
+static int run_cascade(cbct_recon *R, const float *d_g, float *d_f, const int *n_outer, int n_cgls, const Regulariser &reg,
+                       int momentum, void *stream);
+
 extern "C" int cbct_recon_run(cbct_recon *R, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu,
                               int momentum, void *stream) {
     if (!R || !d_g || !d_f || !n_outer || n_cgls < 0 || !(mu >= 0.f)) return CBCT_E_INVALID;
+    return run_cascade(R, d_g, d_f, n_outer, n_cgls, Regulariser{false, mu, 0.f, 0.f, 0}, momentum, stream);
+}
+
+extern "C" int cbct_recon_run_tv(cbct_recon *R, const float *d_g, float *d_f, const int *n_outer, int n_cgls, float mu_tv, float eps,
+                                 int max_rof_iter, float rel_tol, int momentum, void *stream) {
+    if (!R || !d_g || !d_f || !n_outer || n_cgls < 0 || !(mu_tv >= 0.f) || !(eps > 0.f) || max_rof_iter < 0 || !(rel_tol >= 0.f))
+        return CBCT_E_INVALID;
+    for (auto &L : R->lev)
+        if (!L.d_tv_work) return CBCT_E_INVALID;          // created without CBCT_RECON_TV
+    return run_cascade(R, d_g, d_f, n_outer, n_cgls, Regulariser{true, mu_tv, eps, rel_tol, max_rof_iter}, momentum, stream);
+}
+
+static int run_cascade(cbct_recon *R, const float *d_g, float *d_f, const int *n_outer, int n_cgls, const Regulariser &reg,
+                       int momentum, void *stream) {
     cudaStream_t st = as_stream(stream);
     // detector binning: level l's data = block means of level l+1's (finest = d_g), i.e. mg_restrict on [view][v][u]
     for (int l = R->n_levels - 2; l >= 0; --l) {
@@ -123,7 +147,8 @@ extern "C" int cbct_recon_run(cbct_recon *R, const float *d_g, float *d_f, const
             CBCT_TRY(cbct_a2_extrapolate(f_cur, f_prev, L.d_x, coef, n, stream));        // 1. v
             CBCT_TRY(cbct_cgls_init(L.cg, g_l, L.d_x, R->d_r, L.d_p, stream));           // 2. f = CGLS[v]
             for (int m = 0; m < n_cgls; ++m) CBCT_TRY(cbct_cgls_step(L.cg, L.d_x, R->d_r, L.d_p, stream));
-            CBCT_TRY(tf_apply_fused(L.d_x, f_new, mu, 1, L.nx, L.ny, L.nz, stream));     // 3.+4. shrink, clamp
+            if (!reg.tv) CBCT_TRY(tf_apply_fused(L.d_x, f_new, reg.mu, 1, L.nx, L.ny, L.nz, stream));   // 3.+4. shrink, clamp
+            else CBCT_TRY(tv_rof(L.d_x, f_new, L.d_tv_work, reg.mu, reg.eps, reg.max_iter, reg.rel_tol, 1, L.nx, L.ny, L.nz, stream));
             float *tmp = f_prev; f_prev = f_cur; f_cur = f_new; f_new = tmp;
             const double t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t_cur * t_cur));    // 5.
             t_prev = t_cur; t_cur = t_next;

@@ -262,3 +262,31 @@ def recon_run(geom, g, n_levels, n_outer, n_cgls=3, mu=5e-4, momentum=True, bin_
     finally:
         lib().cbct_recon_destroy(h)
     return out
+
+
+def tv_rof(u, mu_tv, eps, max_iter=30, rel_tol=1e-3, clamp=False):
+    """(f, trials, accepted, energy) of tv_rof / tv_rof_result"""
+    nx, ny, nz = _dims(u.shape)
+    out = Buf(u.shape)
+    work = Buf((int(lib().tv_rof_workspace_bytes(nx, ny, nz)),), np.uint8)
+    check(lib().tv_rof(u.ptr, out.ptr, work.ptr, float(mu_tv), float(eps), int(max_iter), float(rel_tol), int(bool(clamp)), nx, ny, nz,
+                       None), "tv_rof")
+    tr, ac, en = C.c_int(), C.c_int(), C.c_double()
+    check(lib().tv_rof_result(work.ptr, nx, ny, nz, C.byref(tr), C.byref(ac), C.byref(en), None), "tv_rof_result")
+    return out, tr.value, ac.value, en.value
+
+
+def recon_run_tv(geom, g, n_levels, n_outer, n_cgls, mu_tv, eps, max_rof_iter, rel_tol, momentum=True):
+    d, keep = cb.make_desc(geom)
+    h = C.c_void_p()
+    check(lib().cbct_recon_create_ex(C.byref(d), int(n_levels), 2, C.byref(h)), "cbct_recon_create_ex")
+    arr = (C.c_int * n_levels)(*[int(v) for v in n_outer])
+    out = Buf((geom.nz, geom.ny, geom.nx))
+    try:
+        check(lib().cbct_recon_run_tv(h, g.ptr, out.ptr, arr, int(n_cgls), float(mu_tv), float(eps), int(max_rof_iter), float(rel_tol),
+                                      int(bool(momentum)), None), "cbct_recon_run_tv")
+        flags = C.c_int(0)
+        check(lib().cbct_recon_status(h, None, C.byref(flags), 0), "cbct_recon_status")
+    finally:
+        lib().cbct_recon_destroy(h)
+    return out

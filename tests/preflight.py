@@ -156,6 +156,14 @@ def main() -> int:
         torch.cuda.synchronize()
         ref = osv.tf_apply(f.astype(np.float64), 0.3, clamp_nonneg=True)
         say(f"tf_apply_fused {shape}", float(np.max(np.abs(d_o.cpu().numpy() - ref)) / np.max(np.abs(f))), 2e-5)
+    from oracle import tv as otv
+    for shape in ((6, 20, 24), (1, 9, 33)):
+        u = (rng.random(shape) + 0.3 * rng.standard_normal(shape)).astype(np.float32)
+        d_u = dev(u)
+        d_o = torch.empty_like(d_u)
+        _, trials, accepted, energy = cb.tv_rof(d_u, d_o, 0.3, 0.05, 25, 1e-3)
+        ref, it = otv.rof(u.astype(np.float64), 0.3, 0.05, 25, 1e-3)
+        say(f"tv_rof {shape} ({trials} trials, oracle {it})", float(np.max(np.abs(d_o.cpu().numpy() - ref)) / np.max(np.abs(ref))) + (0.0 if trials == it else 1.0), 2e-5)
     fine = rng.random((6, 8, 10)).astype(np.float32)
     d_c = torch.empty((6, 4, 5), dtype=torch.float32, device="cuda")
     d_fine = torch.empty((6, 8, 10), dtype=torch.float32, device="cuda")

@@ -19,7 +19,7 @@ def declared_symbols():
     for header in ("cbct.h", "cbct_debug.h"):        # the product ABI and the probes
         text = open(os.path.join(ROOT, "include", header)).read()
         text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-        names += re.findall(r"\b(?:int|long long|const char \*)\s*\*?\s*((?:cbct|tf|mg)_\w+)\s*\(", text)
+        names += re.findall(r"\b(?:int|long long|size_t|const char \*)\s*\*?\s*((?:cbct|tf|tv|mg)_\w+)\s*\(", text)
     return sorted(set(names))
 
 

@@ -149,6 +149,55 @@ def test_short_scan_cascade_with_detector_binning():
     assert sl.lib().cbct_recon_create_ex(C.byref(d), 2, 6, C.byref(h)) == cb.CBCT_E_INVALID      # unknown flag
 
 
+@pytest.mark.parametrize("shape", [(6, 20, 24), (1, 9, 33), (5, 1, 7), (3, 4, 1), (1, 1, 1)])
+def test_tv_rof_matches_oracle(shape):
+    """the ROF descent with its device-resident control state against the oracle's
+    loop -- same number of trials and accepted steps (the decisions are taken on fp64 energies on both sides), same
+    volume, same final energy; ragged and 1-thick shapes; with and without the positivity clamp."""
+    from oracle import tv as otv
+    rng = np.random.default_rng(sum(shape))
+    u = (rng.random(shape) + 0.3 * rng.standard_normal(shape)).astype(np.float32)
+    for mu_tv, eps, max_iter, rel_tol in ((0.3, 0.05, 25, 1e-3), (0.05, 0.02, 8, 0.0), (0.0, 0.05, 5, 1e-3)):
+        trace = []
+        ref, it = otv.rof(u.astype(np.float64), mu_tv, eps, max_iter, rel_tol, trace=trace)
+        out, trials, accepted, energy = sl.tv_rof(sl.dev(u), mu_tv, eps, max_iter, rel_tol)
+        assert trials == it and accepted == sum(1 for t in trace if t[0]), (shape, mu_tv, trials, it)
+        assert np.max(np.abs(out.numpy() - ref)) <= 2e-5 * max(np.max(np.abs(ref)), 1e-30), (shape, mu_tv)
+        e_ref = otv.tv_energy(ref, u.astype(np.float64), mu_tv, eps)
+        assert abs(energy - e_ref) <= 1e-5 * max(e_ref, 1e-30)
+    out, *_ = sl.tv_rof(sl.dev(u), 0.3, 0.05, 25, 1e-3, clamp=True)
+    ref, _ = otv.rof(u.astype(np.float64), 0.3, 0.05, 25, 1e-3)
+    assert np.max(np.abs(out.numpy() - np.maximum(ref, 0.0))) <= 2e-5 * np.max(np.abs(ref))
+    assert "cbct::tv_trial_kernel" in sl.kernel_log()
+
+
+def test_tv_cascade_matches_oracle():
+    """the TV comparison algorithm on the two-level cascade (cbct_recon_run_tv) against solver.multigrid_a2 with the ROF
+    regulariser of oracle/tv.py"""
+    from oracle import tv as otv
+    G = syn.Geometry(32, 32, 8, 4.0, 4.0, 4.0, 48, 16, 3.2, 3.2, 1000.0, 1500.0, tuple(2 * np.pi * k / 12 for k in range(12)))
+    f0 = syn.uniform_volume(G, 83)
+    g = op.forward(G, f0.astype(np.float64)).astype(np.float32)
+
+    def make_ops(fac):
+        return ops(G.coarsen_xy(fac) if fac > 1 else G)
+
+    mu_tv, eps, rof_iter, rel_tol, n_outer, n_cgls = 0.02, 0.01, 10, 1e-3, [2, 2], 2
+    ref = osv.multigrid_a2(make_ops, G.vol_shape, g.astype(np.float64), 2, n_outer, n_cgls, 0.0,
+                           regulariser=otv.tv_regulariser(mu_tv, eps, rof_iter, rel_tol))
+    out = sl.recon_run_tv(G, sl.dev(g), 2, n_outer, n_cgls, mu_tv, eps, rof_iter, rel_tol).numpy()
+    assert rel(out, ref) <= 1e-4
+    import ctypes as C
+    from paper_1008_2042_b200 import binding as cb
+    d, _keep = cb.make_desc(G)                                  # a handle created without CBCT_RECON_TV has no workspace for it
+    h = C.c_void_p()
+    sl.check(sl.lib().cbct_recon_create_ex(C.byref(d), 1, 0, C.byref(h)), "create")
+    arr = (C.c_int * 1)(1)
+    buf = sl.Buf(G.vol_shape)
+    assert sl.lib().cbct_recon_run_tv(h, sl.dev(g).ptr, buf.ptr, arr, 1, 0.1, 0.1, 3, 1e-3, 1, None) == cb.CBCT_E_INVALID
+    sl.lib().cbct_recon_destroy(h)
+
+
 def test_microbench_kernels_stay_in_bounds():
     """cbct_microbench (SURVEY.md §8(d) denominators) with its timed loops shortened: every kernel runs under the shim's
     guards and alignment checks; the rates themselves mean nothing on the host."""

@@ -283,3 +283,47 @@ def test_short_scan_cascade_with_detector_binning():
         assert rec.status() == (True, [])
         assert rel(host(d_f), ref) <= 1e-4, binned
         rec.close()
+
+
+# ------------------------------------------------------------------------------------------ NEXT-3: TV / ROF comparison
+@pytest.mark.parametrize("shape", [(16, 64, 64), (6, 37, 131), (1, 9, 33), (5, 1, 7), (1, 1, 1)])
+def test_tv_rof_matches_oracle(shape):
+    """the ROF gradient descent (device-resident step control) against the
+    oracle's loop: same trials / accepted steps (both sides decide on fp64 energies), same volume, same energy."""
+    from oracle import tv as otv
+    rng = np.random.default_rng(sum(shape))
+    u = (rng.random(shape) + 0.3 * rng.standard_normal(shape)).astype(np.float32)
+    d_u = dev(u)
+    d_f = torch.empty_like(d_u)
+    for mu_tv, eps, max_iter, rel_tol in ((0.3, 0.05, 25, 1e-3), (0.05, 0.02, 8, 0.0), (0.0, 0.05, 5, 1e-3)):
+        trace = []
+        ref, it = otv.rof(u.astype(np.float64), mu_tv, eps, max_iter, rel_tol, trace=trace)
+        _, trials, accepted, energy = cb.tv_rof(d_u, d_f, mu_tv, eps, max_iter, rel_tol)
+        assert trials == it and accepted == sum(1 for t in trace if t[0]), (shape, mu_tv, trials, it)
+        assert np.max(np.abs(host(d_f) - ref)) <= 2e-5 * max(np.max(np.abs(ref)), 1e-30), (shape, mu_tv)
+        e_ref = otv.tv_energy(ref, u.astype(np.float64), mu_tv, eps)
+        assert abs(energy - e_ref) <= 1e-5 * max(e_ref, 1e-30)
+    cb.tv_rof(d_u, d_f, 0.3, 0.05, 25, 1e-3, clamp_nonneg=True)
+    ref, _ = otv.rof(u.astype(np.float64), 0.3, 0.05, 25, 1e-3)
+    assert np.max(np.abs(host(d_f) - np.maximum(ref, 0.0))) <= 2e-5 * np.max(np.abs(ref))
+
+
+def test_tv_cascade_matches_oracle():
+    """cbct_recon_run_tv (the paper's TV comparison algorithm on the multigrid cascade) against solver.multigrid_a2 with
+    the ROF regulariser; config-1 geometry, two levels."""
+    from oracle import tv as otv
+    w, _, f0, g = syn.make_inputs(1)
+    G = w.geometry
+
+    def make_ops(fac):
+        return ops(G.coarsen_xy(fac) if fac > 1 else G)
+
+    mu_tv, eps, rof_iter, rel_tol, n_outer, n_cgls = 2e-3, 1e-3, 10, 1e-3, [2, 2], 2
+    ref = osv.multigrid_a2(make_ops, G.vol_shape, g.astype(np.float64), 2, n_outer, n_cgls, 0.0,
+                           regulariser=otv.tv_regulariser(mu_tv, eps, rof_iter, rel_tol))
+    rec = cb.Recon(G, 2, tv=True)
+    d_f = torch.empty(G.vol_shape, dtype=torch.float32, device="cuda")
+    rec.run_tv(dev(g), d_f, n_outer, n_cgls, mu_tv, eps, rof_iter, rel_tol, True)
+    assert rec.status() == (True, [])
+    assert rel(host(d_f), ref) <= 1e-4
+    rec.close()
