@@ -417,6 +417,8 @@ def main():
     ctx["siddon_p_ms"] = guarded("siddon_forward", lambda: med(lambda: geom.siddon_forward(d_vol, d_proj), 3))
     ctx["siddon_pt_ms"] = guarded("siddon_backproject", lambda: med(lambda: geom.siddon_backproject(d_g, d_tmp), 3))
     ctx["eq3_ms"] = guarded("backproject_eq3", lambda: med(lambda: geom.backproject_eq3(d_g, d_tmp), 3))
+    ctx["tf_fused_tile_ms"] = guarded("tf_apply_fused_tile", lambda: med(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True, impl="tile"), 3))
+    ctx["tf_fused_march_ms"] = guarded("tf_apply_fused_march", lambda: med(lambda: cb.tf_apply_fused(d_vol, d_tmp, MU, True, impl="march"), 3))
     ctx["tf_decompose_ms"] = guarded("tf_decompose", lambda: med(lambda: cb.tf_decompose(d_vol, d_alpha), 3))
     ctx["tf_shrink_ms"] = guarded("tf_shrink", lambda: med(lambda: cb.tf_shrink(d_alpha, MU), 3))
     ctx["tf_reconstruct_ms"] = guarded("tf_reconstruct", lambda: med(lambda: cb.tf_reconstruct(d_alpha, d_tmp), 3))
@@ -485,6 +487,7 @@ def main():
                    full_recon="3-level multigrid, 5/10/15 A2 outer iterations, n_cgls=3, mu=5e-4, device-resident "
                               "(PAPER.md:288 recipe; paper: ~5 min on Tesla C1060)",
                    full_recon_rrms_vs_phantom=rrms,
+                   tf_fused_kernel=guarded("tf_apply_fused_describe", cb.tf_apply_fused_describe),
                    tf_fused_gbs=2 * geom.n_vox * 4 / ms_tf / 1e6, hbm_peak_gbs=hbm["hbm_gbs"], hbm_peak_source=hbm["source"],
                    wall_s_timed_region=t_wall, errors=errors,
                    paper_context="paper: ~2.7-3.5 s per P+P^T pair, ~5 min full recon on Tesla C1060 (PAPER.md:23, :402)"))

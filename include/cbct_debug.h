@@ -33,6 +33,14 @@ int cbct_microbench(int kind, int iters, double out[3], void *stream);
  * kernel behind tf_reconstruct.  Same arguments and result. */
 int tf_reconstruct_direct(const float *d_alpha, float *d_f, int nx, int ny, int nz, void *stream);
 
+/* The two kernels behind tf_apply_fused (include/cbct.h), each on its own: _tile is the 3-D shared-memory tile with
+ * 27-tap sums, _march the z-marching separable kernel that reads every voxel once.  tf_apply_fused uses _march once it
+ * has reproduced _tile on the device in use (one built-in problem, first call of the process; CBCT_TF_FUSED_IMPL =
+ * tile | march forces a choice); _describe names the kernel in use (static storage).  Same arguments and result. */
+int tf_apply_fused_tile(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz, void *stream);
+int tf_apply_fused_march(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz, void *stream);
+const char *tf_apply_fused_describe(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -26,6 +26,7 @@ EXPORTS = [
     "cbct_forward", "cbct_backproject", "cbct_forward_host", "cbct_backproject_host",
     "cbct_backproject_fixed_point_plan", "cbct_backproject_eq3", "cbct_siddon_prepare", "cbct_siddon_forward", "cbct_siddon_backproject",
     "cbct_siddon_fixed_point_plan", "cbct_microbench", "tf_reconstruct_direct",
+    "tf_apply_fused_tile", "tf_apply_fused_march", "tf_apply_fused_describe",
     "cbct_cgls_create", "cbct_cgls_destroy", "cbct_cgls_init", "cbct_cgls_step", "cbct_cgls_scalars",
     "tf_decompose", "tf_shrink", "tf_reconstruct", "tf_apply_fused",
     "mg_restrict", "mg_prolong", "cbct_a2_extrapolate", "tv_rof_workspace_bytes", "tv_rof", "tv_rof_result", "cbct_recon_run_tv",
@@ -104,6 +105,10 @@ def _declare(L):
     L.tf_reconstruct.argtypes = [fp, fp, ip, ip, ip, vp]
     L.tf_reconstruct_direct.argtypes = [fp, fp, ip, ip, ip, vp]
     L.tf_apply_fused.argtypes = [fp, fp, C.c_float, ip, ip, ip, ip, vp]
+    L.tf_apply_fused_tile.argtypes = [fp, fp, C.c_float, ip, ip, ip, ip, vp]
+    L.tf_apply_fused_march.argtypes = [fp, fp, C.c_float, ip, ip, ip, ip, vp]
+    L.tf_apply_fused_describe.restype = C.c_char_p
+    L.tf_apply_fused_describe.argtypes = []
     L.mg_restrict.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
     L.mg_prolong.argtypes = [fp, fp, ip, ip, ip, ip, ip, ip, vp]
     L.cbct_a2_extrapolate.argtypes = [fp, fp, fp, C.c_float, C.c_int64, vp]
@@ -121,7 +126,7 @@ def _declare(L):
     L.cbct_tf_reconstruct.argtypes = [C.POINTER(GeometryDesc), fp, fp, ip, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
     L.cbct_tf_reconstruct_host.argtypes = [C.POINTER(GeometryDesc), fp, fp, ip, C.POINTER(C.c_int), ip, C.c_float, ip, vp]
     for name in EXPORTS:
-        if name != "cbct_status_string":
+        if name not in ("cbct_status_string", "tf_apply_fused_describe"):
             getattr(L, name).restype = C.c_int
     L.cbct_launch_count.restype = C.c_longlong
     L.tv_rof_workspace_bytes.restype = C.c_size_t
@@ -383,11 +388,18 @@ def tf_reconstruct_direct(d_alpha, d_f, stream=None):
     return d_f
 
 
-def tf_apply_fused(d_in, d_out, mu: float, clamp_nonneg: bool = False, stream=None):
+def tf_apply_fused(d_in, d_out, mu: float, clamp_nonneg: bool = False, stream=None, impl: str | None = None):
+    """impl None: the library's choice (tf_apply_fused); "tile" / "march": that kernel on its own (cbct_debug.h)"""
     nx, ny, nz = _dims(d_in.shape)
-    _check(lib().tf_apply_fused(_dptr(d_in), _dptr(d_out, nx * ny * nz), float(mu), int(bool(clamp_nonneg)), nx, ny, nz,
-                                _stream(stream)), "tf_apply_fused")
+    fn = {None: lib().tf_apply_fused, "tile": lib().tf_apply_fused_tile, "march": lib().tf_apply_fused_march}[impl]
+    _check(fn(_dptr(d_in), _dptr(d_out, nx * ny * nz), float(mu), int(bool(clamp_nonneg)), nx, ny, nz, _stream(stream)),
+           "tf_apply_fused")
     return d_out
+
+
+def tf_apply_fused_describe() -> str:
+    """cbct_debug.h: the kernel tf_apply_fused uses in this process"""
+    return lib().tf_apply_fused_describe().decode()
 
 
 def tv_rof(d_u, d_f, mu_tv: float, eps: float, max_iter: int = 30, rel_tol: float = 1e-3, clamp_nonneg: bool = False, stream=None):

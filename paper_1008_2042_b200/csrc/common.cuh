@@ -202,4 +202,5 @@ void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,
                  cudaStream_t st);
 constexpr int kReduceBlocks = 1184;     // 148 SMs x 8
+void tf_fused_prepare();                // decides (once per process) which kernel serves tf_apply_fused; may synchronise the device
 }  // namespace cbct

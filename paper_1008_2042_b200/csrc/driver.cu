@@ -95,6 +95,7 @@ extern "C" int cbct_recon_create_ex(const cbct_geometry_desc *finest, int n_leve
         if (e != cudaSuccess) status = set_cuda_error(e);
     }
     if (status != CBCT_OK) { cbct_recon_destroy(R); return status; }
+    tf_fused_prepare();                                  // the one-off self-check of the fused tight-frame kernel happens here, not in a hot call
     *out = R;
     return CBCT_OK;
 }

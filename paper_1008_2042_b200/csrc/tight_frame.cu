@@ -3,6 +3,12 @@
 // Boundary: edge-replicate extension in D, exact matrix transpose in D^T:
 // for the symmetric filters h0, h2 the transpose is the flipped filter with edge-replicate extension
 // of alpha, for the antisymmetric h1 it is the flipped filter with SIGN-FLIPPED replicate extension.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
 #include "../../include/cbct_debug.h"
 #include "common.cuh"
 
@@ -276,6 +282,157 @@ __global__ void __launch_bounds__(256) tf_fused_kernel(const float *__restrict__
     }
 }
 
+
+// ------------------------------------------------------------------------------ fused [H] D^T T_mu D, z-marching
+// The same result as tf_fused_kernel with every voxel read from global memory once per CTA and no 27-tap sums: the CTA
+// owns a 28(x) x (4 FM_WARPS RPT - 4)(y) column of outputs over a z-segment and walks the planes once.
+//   * ||alpha_h||^2 from SEPARABLE, cancellation-free pieces.  Per axis the three filters satisfy
+//     sum_l (h_l * g)^2 = h0 * g^2  (the identity above, one axis at a time), hence with X_l = h_l *x f, Y_0m = h_m *y X_0,
+//     alpha_00n = h_n *z Y_00:
+//       ||alpha_h||^2 = Wz[ Wy[X_1^2 + X_2^2] + Y_01^2 + Y_02^2 ] + alpha_001^2 + alpha_002^2
+//     (bands with l != 0; bands with l = 0, m != 0; bands with l = m = 0, n != 0): a sum of non-negative terms built
+//     from difference filters, so no local mean has to be subtracted first (what forced tf_fused_kernel's 27-tap form).
+//   * x neighbours by warp shuffle (a warp = 32 consecutive columns of one row, 28 of them outputs), y neighbours
+//     through shared memory (only the first / last row of a thread's RPT rows), z neighbours in rolling registers;
+//   * the synthesis  out = f W0[s] + W0[(1-s) W0 f]  is three more separable [1 2 1]/4 passes with the same plumbing, one
+//     plane behind the analysis; its z-pass is kept as three rolling accumulators per field (plane j adds 1/4, 1/2, 1/4
+//     to the outputs j-1, j, j+1; the planes 0 and nz-1 add their clamped copy to themselves).
+// Extensions are "the value at the clamped position" as in tf_fused_kernel: rows / columns / planes are LOADED at
+// clamped coordinates (so the analysis fields of an outside row equal the face row's), and the synthesis passes take
+// a face voxel's outside neighbour from the voxel itself.
+constexpr int FM_WARPS = 8, FM_TX = 28;
+
+// [1 2 1] and [-1 2 -1] of (m, c, p) WITHOUT the factor 1/4, and the squared antisymmetric tap 2 (p - m)^2 = 16 (h1 * g)^2:
+// the normalisations (powers of two, exact) are applied once per field instead of once per pass.
+__device__ __forceinline__ void fm_pass(float m, float c, float p, float &lo, float &hi, float &d2) {
+    const float e = m + p, d = p - m;
+    lo = fmaf(2.f, c, e);
+    hi = fmaf(2.f, c, -e);
+    d2 = (d + d) * d;
+}
+__device__ __forceinline__ float fm_low(float m, float c, float p) { return fmaf(2.f, c, m + p); }
+
+template <int RPT>
+__global__ void __launch_bounds__(FM_WARPS * 32) tf_fused_march_kernel(const float *__restrict__ fin, float *__restrict__ fout,
+                                                                       float mu, int clamp_nonneg, int nx, int ny, int nz, int zseg) {
+    constexpr int R = FM_WARPS * RPT;                              // rows of the CTA, R - 4 of them outputs
+    __shared__ float sA0[R][32], sA1[R][32];                       // analysis: 4 X_0 and 16 (X_1^2 + X_2^2) of the rows other threads need
+    __shared__ float sS0[R][32], sS1[R][32];                       // synthesis: 4 Wx[s], 4 Wx[b]
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * FM_TX, y0 = blockIdx.y * (R - 4);
+    const int za = blockIdx.z * zseg, zb = min(za + zseg, nz);
+    const int xl = x0 - 2 + lane, r0 = w * RPT;
+    const int lane_m = max(lane - 1, 0), lane_p = min(lane + 1, 31);
+    // synthesis neighbours are "the value at the clamped position": a face voxel's outside neighbour is the voxel itself
+    const int slane_m = xl == 0 ? lane : lane_m, slane_p = xl == nx - 1 ? lane : lane_p;
+    const int plane = nx * ny;                                     // nx ny nz < 2^31 (tf_check): 32-bit element offsets
+    int rowoff[RPT];
+    unsigned face_lo = 0, face_hi = 0, store = 0;                  // bit i: row i is y = 0 / y = ny - 1 / an output of this thread
+#pragma unroll
+    for (int i = 0; i < RPT; ++i) {
+        const int yl = y0 - 2 + r0 + i, r = r0 + i;
+        rowoff[i] = clampi(yl, 0, ny - 1) * nx + clampi(xl, 0, nx - 1);
+        face_lo |= (yl == 0) << i;
+        face_hi |= (yl == ny - 1) << i;
+        store |= (r >= 2 && r < R - 2 && yl < ny && lane >= 2 && lane < 2 + FM_TX && xl < nx) << i;
+    }
+    // shared rows read for the first / last row of this thread (clamped into the CTA; the face rule for the synthesis)
+    const int ra_up = max(r0 - 1, 0), ra_dn = min(r0 + RPT, R - 1);
+    const int rs_up = (face_lo & 1u) ? r0 : ra_up, rs_dn = ((face_hi >> (RPT - 1)) & 1u) ? r0 + RPT - 1 : ra_dn;
+    float c0[RPT], c1[RPT], c2[RPT];                               // f of the planes q, q+1, q+2 (loads two steps ahead)
+    float fa[RPT], fb[RPT], Ya[RPT], Yb[RPT], ta[RPT], tb[RPT];    // f, 16 Y_00, 256 t of the planes q-2, q-1
+    float Sp[RPT], Sc[RPT], Bp[RPT], Bc[RPT];                      // z-pass accumulators of the outputs j-1, j
+#pragma unroll
+    for (int i = 0; i < RPT; ++i) {
+        c0[i] = __ldg(fin + clampi(za - 2, 0, nz - 1) * plane + rowoff[i]);
+        c1[i] = __ldg(fin + clampi(za - 1, 0, nz - 1) * plane + rowoff[i]);
+        c2[i] = __ldg(fin + clampi(za, 0, nz - 1) * plane + rowoff[i]);
+        fa[i] = fb[i] = Ya[i] = Yb[i] = ta[i] = tb[i] = Sp[i] = Sc[i] = Bp[i] = Bc[i] = 0.f;
+    }
+#pragma unroll 3                                                  // the rolling registers are rings of three: no moves
+    for (int q = za - 2; q <= zb + 1; ++q) {                       // CTA-uniform trip count and branches
+        float fn[RPT], X0[RPT], Q1[RPT], Yn[RPT], tn[RPT], Sn[RPT], Bn[RPT];
+#pragma unroll
+        for (int i = 0; i < RPT; ++i) { fn[i] = c0[i]; c0[i] = c1[i]; c1[i] = c2[i]; }
+        if (q + 3 <= zb + 1) {
+            const float *pl = fin + clampi(q + 3, 0, nz - 1) * plane;
+#pragma unroll
+            for (int i = 0; i < RPT; ++i) c2[i] = __ldg(pl + rowoff[i]);
+        }
+        // analysis, x-pass on plane q: X0 = 4 X_0, Q1 = 16 (X_1^2 + X_2^2)
+#pragma unroll
+        for (int i = 0; i < RPT; ++i) {
+            float hi, d2;
+            fm_pass(__shfl_sync(full, fn[i], lane_m), fn[i], __shfl_sync(full, fn[i], lane_p), X0[i], hi, d2);
+            Q1[i] = fmaf(hi, hi, d2);
+        }
+        sA0[r0][lane] = X0[0]; sA1[r0][lane] = Q1[0];
+        if (RPT > 1) { sA0[r0 + RPT - 1][lane] = X0[RPT - 1]; sA1[r0 + RPT - 1][lane] = Q1[RPT - 1]; }
+        __syncthreads();
+        // analysis, y-pass: Yn = 16 Y_00, tn = 256 (Wy[X_1^2 + X_2^2] + Y_01^2 + Y_02^2)
+#pragma unroll
+        for (int i = 0; i < RPT; ++i) {
+            const float X0m = i > 0 ? X0[i - 1] : sA0[ra_up][lane], X0p = i < RPT - 1 ? X0[i + 1] : sA0[ra_dn][lane];
+            const float Q1m = i > 0 ? Q1[i - 1] : sA1[ra_up][lane], Q1p = i < RPT - 1 ? Q1[i + 1] : sA1[ra_dn][lane];
+            float hi, d2;
+            fm_pass(X0m, X0[i], X0p, Yn[i], hi, d2);
+            tn[i] = fmaf(4.f, fm_low(Q1m, Q1[i], Q1p), fmaf(hi, hi, d2));      // 64 Wy[16 q] * 4 + 256 (Y_01^2 + Y_02^2)
+        }
+        // analysis, z-pass on plane j = q - 1 (planes q-2, q-1, q), shrink factor, then the synthesis x-pass
+        const int j = q - 1;
+        const bool vj = j >= 0 && j < nz && j >= za - 1 && j <= zb;
+        float sx[RPT], bx[RPT];
+        if (vj) {
+#pragma unroll
+            for (int i = 0; i < RPT; ++i) {
+                float m64, hi, d2;
+                fm_pass(Ya[i], Yb[i], Yn[i], m64, hi, d2);                      // 64 alpha_000, 64 alpha_002, 4096 alpha_001^2
+                const float Eh = (fmaf(4.f, fm_low(ta[i], tb[i], tn[i]), fmaf(hi, hi, d2))) * (1.f / 4096.f);
+                const float s = shrink_factor(Eh, mu), b = (1.f - s) * (m64 * (1.f / 64.f));
+                sx[i] = fm_low(__shfl_sync(full, s, slane_m), s, __shfl_sync(full, s, slane_p));
+                bx[i] = fm_low(__shfl_sync(full, b, slane_m), b, __shfl_sync(full, b, slane_p));
+            }
+            sS0[r0][lane] = sx[0]; sS1[r0][lane] = bx[0];
+            if (RPT > 1) { sS0[r0 + RPT - 1][lane] = sx[RPT - 1]; sS1[r0 + RPT - 1][lane] = bx[RPT - 1]; }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < RPT; ++i) { Sn[i] = 0.f; Bn[i] = 0.f; }
+        if (vj) {
+            // synthesis, y-pass (sxy = 16 Wy Wx[s]) and the z-pass contributions of plane j (weights 1, 2, 1 and the faces' own copy)
+            const float wc = 2.f + (j == 0 ? 1.f : 0.f) + (j == nz - 1 ? 1.f : 0.f);
+#pragma unroll
+            for (int i = 0; i < RPT; ++i) {
+                float su = i > 0 ? sx[i - 1] : sS0[rs_up][lane], sd = i < RPT - 1 ? sx[i + 1] : sS0[rs_dn][lane];
+                float bu = i > 0 ? bx[i - 1] : sS1[rs_up][lane], bd = i < RPT - 1 ? bx[i + 1] : sS1[rs_dn][lane];
+                if (i > 0 && ((face_lo >> i) & 1u)) { su = sx[i]; bu = bx[i]; }
+                if (i < RPT - 1 && ((face_hi >> i) & 1u)) { sd = sx[i]; bd = bx[i]; }
+                const float sxy = fm_low(su, sx[i], sd), bxy = fm_low(bu, bx[i], bd);
+                Sp[i] += sxy; Sc[i] = fmaf(wc, sxy, Sc[i]); Sn[i] = sxy;
+                Bp[i] += bxy; Bc[i] = fmaf(wc, bxy, Bc[i]); Bn[i] = bxy;
+            }
+        }
+        // output plane q - 2 is complete: out = f W0[s] + W0[b], the accumulators carry the factor 64
+        const int o = q - 2;
+        if (o >= za && o < zb) {
+            float *pl = fout + o * plane;
+#pragma unroll
+            for (int i = 0; i < RPT; ++i)
+                if ((store >> i) & 1u) {
+                    float out = fmaf(fa[i], Sp[i], Bp[i]) * (1.f / 64.f);
+                    if (clamp_nonneg) out = fmaxf(out, 0.f);
+                    pl[rowoff[i]] = out;
+                }
+        }
+#pragma unroll
+        for (int i = 0; i < RPT; ++i) {
+            Sp[i] = Sc[i]; Sc[i] = Sn[i]; Bp[i] = Bc[i]; Bc[i] = Bn[i];
+            Ya[i] = Yb[i]; Yb[i] = Yn[i]; ta[i] = tb[i]; tb[i] = tn[i]; fa[i] = fb[i]; fb[i] = fn[i];
+        }
+    }
+}
+
 }  // namespace cbct
 
 using namespace cbct;
@@ -320,12 +477,99 @@ extern "C" int tf_reconstruct_direct(const float *d_alpha, float *d_f, int nx, i
     return CBCT_OK;
 }
 
+static int launch_tf_fused_tile(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz, cudaStream_t st) {
+    dim3 grid(cdiv(nx, FT_X), cdiv(ny, FT_Y), cdiv(nz, FT_Z));
+    tf_fused_kernel<<<grid, 256, 0, st>>>(d_in, d_out, mu, clamp_nonneg, nx, ny, nz);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+static int launch_tf_fused_march(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz, cudaStream_t st) {
+    const int rpt = ny > 12 ? 4 : 2, rows_out = FM_WARPS * rpt - 4;
+    const int tx = cdiv(nx, FM_TX), ty = cdiv(ny, rows_out);
+    // z-segments: enough CTAs for ~8 per SM, never shorter than 8 planes (a segment recomputes 4 planes of halo)
+    int nseg = (int)((1184.0 + 0.5 * tx * ty) / ((double)tx * ty));
+    nseg = nseg < 1 ? 1 : nseg;
+    if (nseg > nz / 8) nseg = nz / 8 > 0 ? nz / 8 : 1;
+    const int zseg = cdiv(nz, nseg);
+    dim3 grid(tx, ty, cdiv(nz, zseg));
+    if (rpt == 4) tf_fused_march_kernel<4><<<grid, FM_WARPS * 32, 0, st>>>(d_in, d_out, mu, clamp_nonneg, nx, ny, nz, zseg);
+    else tf_fused_march_kernel<2><<<grid, FM_WARPS * 32, 0, st>>>(d_in, d_out, mu, clamp_nonneg, nx, ny, nz, zseg);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+// Which kernel serves tf_apply_fused: decided once per process.  tf_fused_kernel (3-D tile, 27-tap sums) is the variant that
+// has run on a B200 (round 1: 0.50 ms at 512x512x70, shared-memory bound); tf_fused_march_kernel reads every voxel once.
+// As for the projectors (geometry.cu: fast_variants_ok), the newer kernel becomes the default only after it has reproduced
+// the older one on the device in use: both run once on a built-in 45 x 37 x 11 volume (ragged in every tile dimension, both
+// z-segment ends inside), with and without the positivity clamp, and must agree to 1e-5 of max|f|.  CBCT_TF_FUSED_IMPL =
+// tile | march forces a choice (read once).  The check runs inside the first tf_apply_fused / cbct_recon_create of the
+// process and synchronises the device then; no later call does.
+static int g_tf_state = -1;                               // -1 undecided, 0 tile, 1 march (checked), 2 march (forced)
+static std::mutex g_tf_mu;
+
+static bool run_tf_selfcheck() {
+    const int nx = 45, ny = 37, nz = 11;
+    const size_t n = (size_t)nx * ny * nz;
+    std::vector<float> h(n), a(n), b(n);
+    unsigned lcg = 777u;
+    for (auto &v : h) { lcg = lcg * 1664525u + 1013904223u; v = (float)(lcg >> 8) * (1.0f / 16777216.0f) - 0.3f; }
+    float *d_in = nullptr, *d_a = nullptr, *d_b = nullptr;
+    bool ok = cudaMalloc(&d_in, n * 4) == cudaSuccess && cudaMalloc(&d_a, n * 4) == cudaSuccess && cudaMalloc(&d_b, n * 4) == cudaSuccess &&
+              cudaMemcpy(d_in, h.data(), n * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    for (int clamp = 0; ok && clamp < 2; ++clamp) {
+        const float mu = clamp ? 0.25f : 0.1f;
+        ok = launch_tf_fused_tile(d_in, d_a, mu, clamp, nx, ny, nz, nullptr) == CBCT_OK &&
+             launch_tf_fused_march(d_in, d_b, mu, clamp, nx, ny, nz, nullptr) == CBCT_OK && cudaDeviceSynchronize() == cudaSuccess &&
+             cudaMemcpy(a.data(), d_a, n * 4, cudaMemcpyDeviceToHost) == cudaSuccess &&
+             cudaMemcpy(b.data(), d_b, n * 4, cudaMemcpyDeviceToHost) == cudaSuccess;
+        for (size_t i = 0; ok && i < n; ++i) ok = std::fabs(a[i] - b[i]) <= 1e-5f;      // max|f| < 1
+    }
+    if (!ok) (void)cudaGetLastError();
+    cudaFree(d_in); cudaFree(d_a); cudaFree(d_b);
+    return ok;
+}
+
+static int tf_fused_choice() {
+    std::lock_guard<std::mutex> lk(g_tf_mu);
+    if (g_tf_state < 0) {
+        const char *e = getenv("CBCT_TF_FUSED_IMPL");
+        if (e && !strcmp(e, "tile")) g_tf_state = 0;
+        else if (e && !strcmp(e, "march")) g_tf_state = 2;
+        else g_tf_state = run_tf_selfcheck() ? 1 : 0;
+    }
+    return g_tf_state;
+}
+
+namespace cbct {
+void tf_fused_prepare() { (void)tf_fused_choice(); }
+}
+
 extern "C" int tf_apply_fused(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz,
                               void *stream) {
     CBCT_TRY(tf_check(d_in, d_out, nx, ny, nz));
     if (d_in == d_out || !(mu >= 0.f)) return CBCT_E_INVALID;
-    dim3 grid(cdiv(nx, FT_X), cdiv(ny, FT_Y), cdiv(nz, FT_Z));
-    tf_fused_kernel<<<grid, 256, 0, as_stream(stream)>>>(d_in, d_out, mu, clamp_nonneg, nx, ny, nz);
-    CBCT_LAUNCH_CHECK();
-    return CBCT_OK;
+    return tf_fused_choice() ? launch_tf_fused_march(d_in, d_out, mu, clamp_nonneg, nx, ny, nz, as_stream(stream))
+                             : launch_tf_fused_tile(d_in, d_out, mu, clamp_nonneg, nx, ny, nz, as_stream(stream));
+}
+
+// cbct_debug.h: each kernel on its own (cross-checks, A/B timing), and which one tf_apply_fused uses
+extern "C" int tf_apply_fused_tile(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz, void *stream) {
+    CBCT_TRY(tf_check(d_in, d_out, nx, ny, nz));
+    if (d_in == d_out || !(mu >= 0.f)) return CBCT_E_INVALID;
+    return launch_tf_fused_tile(d_in, d_out, mu, clamp_nonneg, nx, ny, nz, as_stream(stream));
+}
+extern "C" int tf_apply_fused_march(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz, void *stream) {
+    CBCT_TRY(tf_check(d_in, d_out, nx, ny, nz));
+    if (d_in == d_out || !(mu >= 0.f)) return CBCT_E_INVALID;
+    return launch_tf_fused_march(d_in, d_out, mu, clamp_nonneg, nx, ny, nz, as_stream(stream));
+}
+extern "C" const char *tf_apply_fused_describe(void) {
+    if (device_supported() != CBCT_OK) return "unavailable (no sm_100 device)";
+    switch (tf_fused_choice()) {
+        case 1: return "tf_fused_march_kernel (self-check passed)";
+        case 2: return "tf_fused_march_kernel (forced)";
+        default: return getenv("CBCT_TF_FUSED_IMPL") ? "tf_fused_kernel (forced)" : "tf_fused_kernel (tf_fused_march_kernel rejected by the self-check)";
+    }
 }

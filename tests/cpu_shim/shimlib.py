@@ -213,9 +213,10 @@ def tf_reconstruct(alpha, direct=False):
     return out
 
 
-def tf_apply_fused(f, mu, clamp):
+def tf_apply_fused(f, mu, clamp, impl=None):
     out = Buf(f.shape)
-    check(lib().tf_apply_fused(f.ptr, out.ptr, float(mu), int(bool(clamp)), *_dims(f.shape), None), "tf_apply_fused")
+    fn = {None: lib().tf_apply_fused, "tile": lib().tf_apply_fused_tile, "march": lib().tf_apply_fused_march}[impl]
+    check(fn(f.ptr, out.ptr, float(mu), int(bool(clamp)), *_dims(f.shape), None), "tf_apply_fused")
     return out
 
 

@@ -134,7 +134,7 @@ def main() -> int:
         h.close()
     # ---- tight frame, multigrid, A2 extrapolation ------------------------------------------------------------------------
     rng = np.random.default_rng(3)
-    for shape in ((16, 64, 64), (5, 7, 9), (1, 33, 40), (6, 37, 131)):
+    for shape in ((16, 64, 64), (5, 7, 9), (1, 33, 40), (6, 37, 131), (40, 30, 29)):
         f = rng.standard_normal(shape).astype(np.float32)
         d_f = dev(f)
         d_a = torch.empty((27,) + shape, dtype=torch.float32, device="cuda")
@@ -152,10 +152,11 @@ def main() -> int:
             fn(d_a, d_o)
             torch.cuda.synchronize()
             say(f"{name} {shape}", float(np.max(np.abs(d_o.cpu().numpy() - r_ref)) / np.max(np.abs(r_ref))))
-        cb.tf_apply_fused(d_f, d_o, 0.3, True)
-        torch.cuda.synchronize()
         ref = osv.tf_apply(f.astype(np.float64), 0.3, clamp_nonneg=True)
-        say(f"tf_apply_fused {shape}", float(np.max(np.abs(d_o.cpu().numpy() - ref)) / np.max(np.abs(f))), 2e-5)
+        for impl in ("tile", "march", None):                  # each kernel on its own, then the library's choice
+            cb.tf_apply_fused(d_f, d_o, 0.3, True, impl=impl)
+            torch.cuda.synchronize()
+            say(f"tf_apply_fused[{impl or cb.tf_apply_fused_describe()}] {shape}", float(np.max(np.abs(d_o.cpu().numpy() - ref)) / np.max(np.abs(f))), 2e-5)
     from oracle import tv as otv
     for shape in ((6, 20, 24), (1, 9, 33)):
         u = (rng.random(shape) + 0.3 * rng.standard_normal(shape)).astype(np.float32)

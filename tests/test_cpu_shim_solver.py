@@ -88,13 +88,48 @@ def test_tf_reconstruct_both_kernels(shape, impl):
     assert np.max(np.abs(out - r_ref)) <= 1e-5 * np.max(np.abs(r_ref))
 
 
-@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("impl", ["tile", "march"])
+@pytest.mark.parametrize("shape", SHAPES + [(70, 57, 29), (23, 13, 57)])       # + several z-segments, several tiles in x and y
 @pytest.mark.parametrize("mu,clamp", [(0.0, False), (0.3, False), (0.3, True), (2.0, True), (1e6, False)])
-def test_tf_fused_matches_oracle(shape, mu, clamp):
+def test_tf_fused_matches_oracle(shape, mu, clamp, impl):
+    """both kernels behind tf_apply_fused (the 3-D tile with 27-tap sums, the separable z-marching one), each on its own"""
     rng = np.random.default_rng(sum(shape) + 1)
     f = rng.standard_normal(shape).astype(np.float32)
     ref = osv.tf_apply(f.astype(np.float64), mu, clamp_nonneg=clamp)
-    assert np.max(np.abs(sl.tf_apply_fused(sl.dev(f), mu, clamp).numpy() - ref)) <= 2e-5 * np.max(np.abs(f))
+    out = sl.tf_apply_fused(sl.dev(f), mu, clamp, impl=impl).numpy()
+    assert sl.kernel_log()[-1].startswith("cbct::tf_fused_march_kernel" if impl == "march" else "cbct::tf_fused_kernel")
+    assert np.max(np.abs(out - ref)) <= 2e-5 * np.max(np.abs(f))
+
+
+@pytest.mark.parametrize("impl", ["tile", "march"])
+def test_tf_fused_on_a_large_offset(impl):
+    """||alpha_h||^2 must not be formed as a difference of large numbers: a flat region of value 100 with noise 0.01 next
+    to an edge (the tile kernel subtracts the centre voxel first, the marching kernel sums squared difference bands)"""
+    rng = np.random.default_rng(5)
+    f = (100.0 + 0.01 * rng.standard_normal((12, 40, 50))).astype(np.float32)
+    f[:, 20:, :] += 50.0
+    ref = osv.tf_apply(f.astype(np.float64), 0.01, clamp_nonneg=True)
+    assert np.max(np.abs(ref - f)) > 1e-4 * np.max(np.abs(f))                  # the shrinkage does something here
+    assert np.max(np.abs(sl.tf_apply_fused(sl.dev(f), 0.01, True, impl=impl).numpy() - ref)) <= 1e-6 * np.max(np.abs(f))
+
+
+@pytest.mark.parametrize("impl", ["tile", "march"])
+def test_tf_fused_on_phantom_with_paper_mu(impl):
+    """piecewise-constant phantom, mu = 5e-4: flat regions sit exactly at ||alpha_h|| = 0"""
+    w, _, f0, _ = syn.make_inputs(1)
+    ref = osv.tf_apply(f0.astype(np.float64), 5e-4, clamp_nonneg=True)
+    out = sl.tf_apply_fused(sl.dev(f0), 5e-4, True, impl=impl).numpy()
+    assert rel(out, ref) <= 1e-5 and np.max(np.abs(out - ref)) <= 1e-5 * np.max(np.abs(f0))
+
+
+def test_tf_fused_default_is_the_checked_marching_kernel():
+    """tf_apply_fused itself: the library's create-time style self-check (march against tile on a built-in volume) runs on
+    the first call and, passing, selects the marching kernel"""
+    f = np.random.default_rng(2).standard_normal((9, 31, 45)).astype(np.float32)
+    out = sl.tf_apply_fused(sl.dev(f), 0.2, True).numpy()
+    assert sl.kernel_log()[-1].startswith("cbct::tf_fused_march_kernel")
+    assert sl.lib().tf_apply_fused_describe().decode().startswith("tf_fused_march_kernel (self-check passed)")
+    assert np.max(np.abs(out - osv.tf_apply(f.astype(np.float64), 0.2, clamp_nonneg=True))) <= 2e-5 * np.max(np.abs(f))
 
 
 @pytest.mark.parametrize("shape,fac", [((6, 8, 10), (2, 2, 1)), ((4, 6, 2), (2, 2, 2)), ((70, 64, 32), (2, 2, 1)),

@@ -167,26 +167,46 @@ def test_tf_reconstruct_both_kernels(shape, impl):
     assert np.max(np.abs(host(d_out) - r_ref)) <= 1e-5 * np.max(np.abs(r_ref))
 
 
-@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("impl", [None, "tile", "march"])
+@pytest.mark.parametrize("shape", SHAPES + [(70, 57, 29), (23, 13, 57)])       # + several z-segments, several tiles in x and y
 @pytest.mark.parametrize("mu,clamp", [(0.0, False), (0.3, False), (0.3, True), (2.0, True), (1e6, False)])
-def test_tf_fused_matches_oracle(shape, mu, clamp):
+def test_tf_fused_matches_oracle(shape, mu, clamp, impl):
+    """tf_apply_fused (the library's choice) and each of the two kernels behind it on its own (cbct_debug.h)"""
     rng = np.random.default_rng(sum(shape) + 1)
     f = rng.standard_normal(shape).astype(np.float32)
     ref = osv.tf_apply(f.astype(np.float64), mu, clamp_nonneg=clamp)
     d_out = torch.empty(shape, dtype=torch.float32, device="cuda")
-    cb.tf_apply_fused(dev(f), d_out, mu, clamp)
+    cb.tf_apply_fused(dev(f), d_out, mu, clamp, impl=impl)
     assert np.max(np.abs(host(d_out) - ref)) <= 2e-5 * np.max(np.abs(f))
 
 
-def test_tf_fused_on_phantom_with_paper_mu():
+@pytest.mark.parametrize("impl", [None, "tile", "march"])
+def test_tf_fused_on_phantom_with_paper_mu(impl):
     """A piecewise-constant phantom with small values and mu = 5e-4: flat regions sit
     exactly at ||alpha_h|| = 0 and edges far above mu."""
     w, _, f0, _ = syn.make_inputs(1)
     ref = osv.tf_apply(f0.astype(np.float64), 5e-4, clamp_nonneg=True)
     d_out = torch.empty(f0.shape, dtype=torch.float32, device="cuda")
-    cb.tf_apply_fused(dev(f0), d_out, 5e-4, True)
+    cb.tf_apply_fused(dev(f0), d_out, 5e-4, True, impl=impl)
     assert rel(host(d_out), ref) <= 1e-5
     assert np.max(np.abs(host(d_out) - ref)) <= 1e-5 * np.max(np.abs(f0))
+
+
+@pytest.mark.parametrize("impl", ["tile", "march"])
+def test_tf_fused_on_a_large_offset(impl):
+    """||alpha_h||^2 must not be formed as a difference of large numbers (value 100, noise 0.01, next to an edge)"""
+    rng = np.random.default_rng(5)
+    f = (100.0 + 0.01 * rng.standard_normal((12, 40, 50))).astype(np.float32)
+    f[:, 20:, :] += 50.0
+    ref = osv.tf_apply(f.astype(np.float64), 0.01, clamp_nonneg=True)
+    d_out = torch.empty(f.shape, dtype=torch.float32, device="cuda")
+    cb.tf_apply_fused(dev(f), d_out, 0.01, True, impl=impl)
+    assert np.max(np.abs(host(d_out) - ref)) <= 1e-6 * np.max(np.abs(f))
+
+
+def test_tf_fused_kernel_in_use_is_reported():
+    print("tf_apply_fused:", cb.tf_apply_fused_describe())
+    assert cb.tf_apply_fused_describe().startswith(("tf_fused_march_kernel", "tf_fused_kernel"))
 
 
 # ------------------------------------------------------------------------------------------ multigrid + A2 step 1
