@@ -30,6 +30,7 @@
  *       CBCT_FORWARD_IMPL = tma | tiled | global      CBCT_BACKPROJECT_IMPL = scatter | cell | gather
  *       CBCT_FW_PACKED = 0|1   CBCT_BT_PACKED = 0|1   (packed fp32-pair or scalar instruction stream)
  *       CBCT_BT_LANES = 0|1    (lane layout of the scatter kernel)
+ *     (tf_apply_fused has a process-wide selection of the same kind, CBCT_TF_FUSED_IMPL: see there.)
  *     A forced implementation that the geometry cannot use makes cbct_geometry_create fail (CBCT_E_UNSUPPORTED);
  *     nothing falls back silently at launch time.
  */
@@ -208,7 +209,12 @@ int tf_shrink(float *d_alpha, float mu, int nx, int ny, int nz, void *stream);
 /* f = D^T alpha = sum_i psi_i(-x) (*) alpha_i. */
 int tf_reconstruct(const float *d_alpha, float *d_f, int nx, int ny, int nz, void *stream);
 /* f_out = [H] D^T T_mu D f_in without materialising alpha (H = max(.,0), PAPER.md:131,
- * applied when clamp_nonneg != 0).  d_in != d_out. */
+ * applied when clamp_nonneg != 0).  d_in != d_out.
+ * Two kernels compute it (cbct_debug.h exposes each): a 3-D shared-memory tile and a z-marching separable one that
+ * reads every voxel once.  The marching kernel serves this call once it has reproduced the tile kernel on the device in
+ * use; that one-off check (a 45x37x11 built-in volume) runs inside the first call of the process -- or earlier, inside
+ * cbct_recon_create -- and synchronises the device then; no later call does.  CBCT_TF_FUSED_IMPL = tile | march (read
+ * once, at that point) forces a choice. */
 int tf_apply_fused(const float *d_in, float *d_out, float mu, int clamp_nonneg, int nx, int ny, int nz,
                    void *stream);
 
