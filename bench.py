@@ -163,6 +163,8 @@ def main():
     ap.add_argument("--peaks", action="store_true", help="run the library's micro-benchmarks (cbct_microbench) and exit")
     ap.add_argument("--no-full-recon", action="store_true", help="skip the one-off 3-level 5/10/15 reconstruction timing")
     ap.add_argument("--no-variants", action="store_true", help="skip the A/B timings of the other kernel variants")
+    ap.add_argument("--full-recon-outer", default="5,10,15",
+                    help="A2 outer iterations per level (coarse to fine) of the one-off full reconstruction; PAPER.md:288: 5,10,15")
     args = ap.parse_args()
 
     from paper_1008_2042_b200 import replicas
@@ -428,6 +430,9 @@ def main():
 
     # ---- the paper's full reconstruction, end to end (context number; 3 levels, 5/10/15) ----
     full_recon_s, rrms = None, None
+    n_outer_full = [int(v) for v in args.full_recon_outer.split(",")]
+    if len(n_outer_full) != 3 or min(n_outer_full) < 0:
+        raise SystemExit("--full-recon-outer takes three non-negative counts, coarse to fine")
     if not args.no_full_recon:
         def full():
             rec3 = cb.Recon(G, 3)
@@ -435,7 +440,7 @@ def main():
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record()
-            rec3.run(d_g, d_f, [5, 10, 15], N_CGLS, MU, True)
+            rec3.run(d_g, d_f, n_outer_full, N_CGLS, MU, True)
             b.record()
             torch.cuda.synchronize()
             ok3, bits3 = rec3.status()
@@ -484,7 +489,7 @@ def main():
                                         "(vector kernels add < 2 %); standalone = the two kernels timed alone after an L2 flush",
                    variants=variants, context_ms=ctx, microbench=peaks,
                    full_recon_s=full_recon_s,
-                   full_recon="3-level multigrid, 5/10/15 A2 outer iterations, n_cgls=3, mu=5e-4, device-resident "
+                   full_recon=f"3-level multigrid, {'/'.join(map(str, n_outer_full))} A2 outer iterations, n_cgls=3, mu=5e-4, device-resident "
                               "(PAPER.md:288 recipe; paper: ~5 min on Tesla C1060)",
                    full_recon_rrms_vs_phantom=rrms,
                    tf_fused_kernel=guarded("tf_apply_fused_describe", cb.tf_apply_fused_describe),

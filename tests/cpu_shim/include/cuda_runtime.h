@@ -10,6 +10,7 @@
 
 #include <cmath>
 #include <cstdlib>
+#include <chrono>
 #include <cstring>
 #include <functional>
 #include <tuple>
@@ -82,11 +83,21 @@ static inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSucce
 static inline cudaError_t cudaDeviceSynchronize() { return cudaSuccess; }
 static inline cudaError_t cudaGetDevice(int *d) { *d = 0; return cudaSuccess; }
 static inline cudaError_t cudaDeviceGetAttribute(int *v, cudaDeviceAttr, int) { *v = 10; return cudaSuccess; }
-static inline cudaError_t cudaEventCreate(cudaEvent_t *e) { *e = nullptr; return cudaSuccess; }
-static inline cudaError_t cudaEventDestroy(cudaEvent_t) { return cudaSuccess; }
-static inline cudaError_t cudaEventRecord(cudaEvent_t, cudaStream_t = nullptr) { return cudaSuccess; }
+// events are wall-clock timestamps: every launch is synchronous here, so "device time between two events" is host time
+struct shim_event { double ms; };
+static inline cudaError_t cudaEventCreate(cudaEvent_t *e) { *e = new shim_event{0.0}; return cudaSuccess; }
+static inline cudaError_t cudaEventDestroy(cudaEvent_t e) { delete e; return cudaSuccess; }
+static inline cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t = nullptr) {
+    if (!e) return cudaErrorInvalidValue;
+    e->ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count();
+    return cudaSuccess;
+}
 static inline cudaError_t cudaEventSynchronize(cudaEvent_t) { return cudaSuccess; }
-static inline cudaError_t cudaEventElapsedTime(float *ms, cudaEvent_t, cudaEvent_t) { *ms = 0.f; return cudaSuccess; }
+static inline cudaError_t cudaEventElapsedTime(float *ms, cudaEvent_t a, cudaEvent_t b) {
+    if (!a || !b) return cudaErrorInvalidValue;
+    *ms = (float)(b->ms - a->ms);
+    return cudaSuccess;
+}
 cudaError_t cudaFuncSetAttribute(const void *func, cudaFuncAttribute, int value);   // records the opt-in per kernel
 template <class F>
 static inline cudaError_t cudaFuncSetAttribute(F *func, cudaFuncAttribute a, int value) {
