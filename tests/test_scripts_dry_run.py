@@ -62,3 +62,19 @@ def test_preflight_runs_to_its_last_line(monkeypatch, capsys):
         assert preflight.main() == 0
     out = capsys.readouterr().out
     assert "preflight ok" in out and "FAIL" not in out
+
+
+def test_gpu_marked_tests_run_under_the_harness():
+    """`--shim-as-cuda` (tests/conftest.py) runs the -m gpu tests themselves on the host.  A quick subset here keeps the
+    option alive; the whole of tests/test_gpu_solver.py and the cfg 1-2 part of tests/test_gpu_projectors.py take ~15 min:
+        python -m pytest tests/test_gpu_solver.py tests/test_gpu_projectors.py -m gpu --shim-as-cuda \\
+            -k "not full_size and not paper_size and not headroom_bound" """
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_gpu_solver.py", "tests/test_gpu_projectors.py", "-m", "gpu",
+                        "--shim-as-cuda", "-q", "-x", "-k",
+                        "mg_restrict or a2_extrapolate or breakdown or tv_rof or degenerate or host_buffer or ragged or geometry_info"],
+                       cwd=root, capture_output=True, text=True, timeout=1200)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
+    assert " passed" in r.stdout and "failed" not in r.stdout
