@@ -17,7 +17,7 @@ __device__ __forceinline__ bool aligned16(const void *a, const void *b = nullptr
 
 enum { S_GAMMA = 0, S_QQ = 1, S_ALPHA = 2, S_BETA = 3, S_RR = 4, S_GAMMA_NEW = 5, S_COUNT = 8 };
 
-// ||v||^2 -> *out.  Block partials in fp64, the last block to finish sums them in index order.
+// ||v||^2 -> *out.  Block partials in fp64, summed by the last block to finish in a fixed order (common.cuh: ordered_total).
 __global__ void __launch_bounds__(256) sumsq_kernel(const float *__restrict__ v, long long n, double *out,
                                                     double *partials, unsigned int *counter) {
     double acc = 0.0;
@@ -30,27 +30,10 @@ __global__ void __launch_bounds__(256) sumsq_kernel(const float *__restrict__ v,
     for (long long i = (n4 << 2) + blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x)
         acc += (double)v[i] * v[i];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     __shared__ double sh[8];
     __shared__ bool last;
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double s = 0.0;
-        for (int w = 0; w < 8; ++w) s += sh[w];
-        partials[blockIdx.x] = s;
-        __threadfence();
-        last = (atomicAdd(counter, 1u) == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (last && threadIdx.x == 0) {
-        __threadfence();
-        double s = 0.0;
-        for (unsigned b = 0; b < gridDim.x; ++b) s += ((volatile double *)partials)[b];
-        *out = s;
-        *counter = 0;
-    }
+    double total;
+    if (ordered_total(acc, partials, counter, sh, &last, total)) *out = total;
 }
 
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,

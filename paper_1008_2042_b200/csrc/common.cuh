@@ -86,6 +86,41 @@ __device__ __forceinline__ void ray_setup(const DevGeom &g, int view, int iv, in
     r.bx = (float)bxd; r.by = (float)byd; r.bz = (float)bzd;
 }
 
+// ---- deterministic two-level fp64 reduction (256-thread blocks) ---------------------------------------------------------
+// Every thread brings its partial sum `acc`; the block's total goes to partials[blockIdx.x]; the block that finishes last
+// adds up all block totals and thread 0 of that block gets the result (return value true, `total` set, counter reset).
+// The order of every addition is fixed by (gridDim, blockDim) alone, so the result is reproducible; the last step is
+// done by the whole block (thread t takes partials t, t + 256, ..., then the same warp / block tree), not by one thread
+// walking gridDim.x dependent loads from L2 -- with 1184 blocks that walk was most of the kernel's time in round 1.
+// `sh` = 8 doubles and `last` = one bool of shared memory, both declared by the calling kernel.
+__device__ __forceinline__ bool ordered_total(double acc, double *partials, unsigned int *counter, double *sh, bool *last, double &total) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += sh[w];
+        partials[blockIdx.x] = s;
+        __threadfence();
+        *last = (atomicAdd(counter, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!*last) return false;                                    // block-uniform
+    __threadfence();
+    double s = 0.0;
+    for (unsigned b = threadIdx.x; b < gridDim.x; b += blockDim.x) s += ((volatile double *)partials)[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;       // thread 0 read sh before the barrier above: no hazard
+    __syncthreads();
+    if (threadIdx.x != 0) return false;
+    total = 0.0;
+    for (int w = 0; w < 8; ++w) total += sh[w];
+    *counter = 0u;
+    return true;
+}
+
 // ---- P^T (cell-driven) tables, built in fp64 at geometry create, stored fp32 ------------------------
 // With r = t / L(u,v) (t = distance from the source) a ray is  X = Kx + Ax r,  Y = Ky + Ay r,  Z = Kz + vz r,
 // so clipping against a cell is done in r and only then scaled by L.  Sample positions use the

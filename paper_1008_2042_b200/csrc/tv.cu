@@ -57,26 +57,11 @@ __global__ void __launch_bounds__(256) tv_energy_kernel(const float *__restrict_
         const float d = __ldg(f + i) - __ldg(u + i);
         acc += (double)d * d + (double)mu * (double)sqrtf(fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, eps2))));
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     __shared__ double sh[8];
     __shared__ bool last;
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int w = 0; w < 8; ++w) t += sh[w];
-        partials[blockIdx.x] = t;
-        __threadfence();
-        last = (atomicAdd(&s->counter, 1u) == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (last && threadIdx.x == 0) {
-        __threadfence();
-        double t = 0.0;
-        for (unsigned b = 0; b < gridDim.x; ++b) t += ((volatile double *)partials)[b];
+    double t;
+    if (ordered_total(acc, partials, &s->counter, sh, &last, t)) {
         if (which) s->Et = t; else { s->E = t; if (t == 0.0) s->done = 1; }       // E(u) = 0: nothing to do (T6)
-        s->counter = 0u;
     }
 }
 

@@ -211,7 +211,10 @@ def test_tf_fused_kernel_in_use_is_reported():
 
 # ------------------------------------------------------------------------------------------ multigrid + A2 step 1
 @pytest.mark.parametrize("shape,fac", [((6, 8, 10), (2, 2, 1)), ((4, 6, 2), (2, 2, 2)), ((70, 64, 32), (2, 2, 1)),
-                                       ((3, 5, 8), (2, 1, 1)), ((2, 2, 2), (1, 1, 2))])
+                                       ((3, 5, 8), (2, 1, 1)), ((2, 2, 2), (1, 1, 2)),
+                                       # rows of float4 (the vectorised kernels): every factor combination, ragged tiles
+                                       ((4, 6, 16), (2, 2, 2)), ((6, 4, 24), (1, 2, 1)), ((2, 6, 8), (2, 1, 2)), ((3, 5, 12), (1, 1, 1)),
+                                       ((66, 18, 264), (2, 2, 2)), ((5, 34, 136), (2, 2, 1))])
 def test_mg_restrict_prolong(shape, fac):
     fx, fy, fz = fac
     rng = np.random.default_rng(5)
