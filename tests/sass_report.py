@@ -1,6 +1,7 @@
 """Instruction mix of the hot loops of the projector kernels, from the SASS of the built objects (no GPU needed).
 
     python tests/sass_report.py            # markdown table on stdout   (TEST TOOLING: tests/test_sass_budget.py is its user)
+    python tests/sass_report.py --resources   # registers / shared memory / Blackwell-specific opcodes per kernel of the built library
 
 For every instantiation of forward_tma_kernel / backproject_scatter_kernel / the Siddon kernels in
 paper_1008_2042_b200/build/*.o it finds the innermost loop that contains the kernel's shared-memory loads (LDS), shared
@@ -45,7 +46,35 @@ def loops(func_text: str, marker: str):
     return best
 
 
+def resources() -> int:
+    """registers, static shared memory and the opcodes that show a Blackwell-native kernel (B200_PROFILING.md: UTMALDG /
+    UTMAREDG = TMA tensor copy / reduction, SYNCS = mbarrier, FFMA2 / FADD2 / FMUL2 = packed fp32 pairs, ATOMS = shared-memory
+    atomics), per kernel of libcbct_b200.so; template instantiations that differ only in box pitches share a row"""
+    lib = os.path.join(HERE, "libcbct_b200.so")
+    usage = subprocess.run(["cuobjdump", "--dump-resource-usage", lib], capture_output=True, text=True).stdout
+    res = {}
+    for m in re.finditer(r"Function (\S+):\n\s*REG:(\d+).*?SHARED:(\d+)", usage):
+        res[m.group(1)] = (int(m.group(2)), int(m.group(3)))
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True).stdout
+    ops = ("UTMALDG", "UTMAREDG", "SYNCS", "FFMA2", "FADD2", "FMUL2", "ATOMS.ADD", "LDS", "REDG", "BAR")
+    rows = {}
+    for chunk in re.split(r"\n\s*Function : ", sass)[1:]:
+        mangled = chunk.split("\n")[0].strip()
+        name = re.sub(r"<\d+, \d+", "<BF, BS", demangle(mangled).replace("cbct::", "").replace("void ", ""))
+        body = [re.sub(r"/\*.*?\*/", "", l).strip() for l in chunk.split("\n") if re.match(r"\s+/\*[0-9a-f]{4}\*/", l)]
+        cnt = tuple(sum(1 for x in body if re.search(r"\b" + re.escape(o), x)) for o in ops)
+        key = (name,) + res.get(mangled, (0, 0)) + cnt
+        rows[key] = rows.get(key, 0) + 1
+    print("| kernel | instantiations | registers | static smem B | " + " | ".join(ops) + " |")
+    print("|---|---|---|---|" + "---|" * len(ops))
+    for key in sorted(rows):
+        print(f"| `{key[0]}` | {rows[key]} | {key[1]} | {key[2]} | " + " | ".join(str(v) for v in key[3:]) + " |")
+    return 0
+
+
 def main() -> int:
+    if "--resources" in sys.argv:
+        return resources()
     rows = []
     for obj in sorted(glob.glob(os.path.join(HERE, "build", "*.o"))):
         sass = subprocess.run(["cuobjdump", "-sass", obj], capture_output=True, text=True).stdout
