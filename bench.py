@@ -311,6 +311,8 @@ def main():
     if rank != 0:
         replicas.shutdown()
         return
+    if world > 1:                                            # context numbers belong to the 1-GPU line; keep the scaling runs short
+        args.no_variants = args.no_full_recon = True
 
     errors = []
 
@@ -453,7 +455,7 @@ def main():
         full_recon_s, rrms = guarded("full reconstruction", full, (None, None))
 
     cpu_baseline = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:              # the oracle is timed beside the 1-GPU number only
         r = time_oracle_sample(G, f0, g, [G.n_views // 3])
         cpu_baseline = dict(value=r["samples"] / r["seconds"] / 1e9, unit=UNIT, cores=omp_threads(), kind="oracle",
                             sample=f"oracle P + P^T (fp64, scatter form) on 1 of {G.n_views} views of the same workload: "
