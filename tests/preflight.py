@@ -165,14 +165,17 @@ def main() -> int:
         _, trials, accepted, energy = cb.tv_rof(d_u, d_o, 0.3, 0.05, 25, 1e-3)
         ref, it = otv.rof(u.astype(np.float64), 0.3, 0.05, 25, 1e-3)
         say(f"tv_rof {shape} ({trials} trials, oracle {it})", float(np.max(np.abs(d_o.cpu().numpy() - ref)) / np.max(np.abs(ref))) + (0.0 if trials == it else 1.0), 2e-5)
-    fine = rng.random((6, 8, 10)).astype(np.float32)
-    d_c = torch.empty((6, 4, 5), dtype=torch.float32, device="cuda")
-    d_fine = torch.empty((6, 8, 10), dtype=torch.float32, device="cuda")
-    cb.mg_restrict(dev(fine), d_c)
-    cb.mg_prolong(d_c, d_fine)
-    torch.cuda.synchronize()
-    say("mg_restrict", float(np.max(np.abs(d_c.cpu().numpy() - osv.mg_restrict(fine.astype(np.float64))))), 1e-6)
-    say("mg_prolong", float(np.max(np.abs(d_fine.cpu().numpy() - osv.mg_prolong(d_c.cpu().numpy().astype(np.float64))))), 1e-6)
+    # scalar kernels (ragged rows) and the float4 kernels (rows of whole float4s), every factor pattern the driver uses
+    for shape, (fx, fy, fz) in (((6, 8, 10), (2, 2, 1)), ((4, 6, 16), (2, 2, 2)), ((6, 4, 24), (1, 2, 1)), ((5, 34, 136), (2, 2, 1))):
+        fine = rng.random(shape).astype(np.float32)
+        d_c = torch.empty((shape[0] // fz, shape[1] // fy, shape[2] // fx), dtype=torch.float32, device="cuda")
+        d_fine = torch.empty(shape, dtype=torch.float32, device="cuda")
+        cb.mg_restrict(dev(fine), d_c, fx, fy, fz)
+        cb.mg_prolong(d_c, d_fine, fx, fy, fz)
+        torch.cuda.synchronize()
+        say(f"mg_restrict {shape} /{fx}{fy}{fz}", float(np.max(np.abs(d_c.cpu().numpy() - osv.mg_restrict(fine.astype(np.float64), fx, fy, fz)))), 1e-6)
+        say(f"mg_prolong  {shape} x{fx}{fy}{fz}",
+            float(np.max(np.abs(d_fine.cpu().numpy() - osv.mg_prolong(d_c.cpu().numpy().astype(np.float64), fx, fy, fz)))), 1e-6)
     # ---- CGLS + the A2 driver (default kernels) ---------------------------------------------------------------------------
     w, _e, f0, g = syn.make_inputs(1)
     G = w.geometry
