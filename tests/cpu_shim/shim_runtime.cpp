@@ -340,8 +340,8 @@ static void complete_warp(Worker *w, int warp) {
     }
     if (!waiting || waiting < alive) return;
     const Fiber &first = *[&]() { for (int i = lo; i < hi; ++i) if (w->fibers[i].state == WAIT_WARP) return &w->fibers[i]; return (Fiber *)nullptr; }();
-    int64_t smin = INT64_MAX, smax = INT64_MIN, sadd = 0;
-    uint64_t umax = 0, umin = UINT64_MAX, ballot = 0;
+    int64_t smin = INT64_MAX, smax = INT64_MIN;
+    uint64_t umax = 0, umin = UINT64_MAX, ballot = 0, sadd = 0;      // sadd wraps (payloads of other collectives are arbitrary bits)
     for (int i = lo; i < hi; ++i) {
         Fiber &g = w->fibers[i];
         if (g.state != WAIT_WARP) continue;
@@ -351,7 +351,7 @@ static void complete_warp(Worker *w, int warp) {
             return;
         }
         const int64_t s = (int64_t)g.wpayload;
-        smin = std::min(smin, s); smax = std::max(smax, s); sadd += s;
+        smin = std::min(smin, s); smax = std::max(smax, s); sadd += (uint64_t)s;
         umax = std::max(umax, g.wpayload); umin = std::min(umin, g.wpayload);
         if (g.wpayload) ballot |= 1ull << (i - lo);
     }
@@ -362,7 +362,7 @@ static void complete_warp(Worker *w, int warp) {
         switch (g.wop) {
             case W_MIN_S32: g.wresult = (uint64_t)smin; break;
             case W_MAX_S32: g.wresult = (uint64_t)smax; break;
-            case W_ADD_S32: g.wresult = (uint64_t)sadd; break;
+            case W_ADD_S32: g.wresult = sadd; break;
             case W_MAX_U32: g.wresult = umax; break;
             case W_MIN_U32: g.wresult = umin; break;
             case W_BALLOT: g.wresult = ballot; break;
