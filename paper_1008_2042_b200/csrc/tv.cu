@@ -48,14 +48,19 @@ __global__ void __launch_bounds__(256) tv_energy_kernel(const float *__restrict_
                                                         int nx, int ny, int nz, double *partials) {
     if (s->done) return;
     const float *f = ((s->cur ^ which) & 1) ? buf1 : buf0;
-    const long long n = (long long)nx * ny * nz;
     double acc = 0.0;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((long long)nx * ny));
-        float gx, gy, gz, inv;
-        tv_diffs(f, x, y, z, nx, ny, nz, eps2, gx, gy, gz, inv);
-        const float d = __ldg(f + i) - __ldg(u + i);
-        acc += (double)d * d + (double)mu * (double)sqrtf(fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, eps2))));
+    // linear block index -> (row tile, plane): 256 threads = 32 (x) x 8 (y), x strides over the row, blocks stride over (y-tile, z)
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, ytiles = (ny + 7) >> 3;
+    for (int job = blockIdx.x; job < ytiles * nz; job += gridDim.x) {
+        const int z = job / ytiles, y = (job - z * ytiles) * 8 + ty;
+        if (y >= ny) continue;
+        const size_t row = ((size_t)z * ny + y) * nx;
+        for (int x = tx; x < nx; x += 32) {
+            float gx, gy, gz, inv;
+            tv_diffs(f, x, y, z, nx, ny, nz, eps2, gx, gy, gz, inv);
+            const float d = __ldg(f + row + x) - __ldg(u + row + x);
+            acc += (double)d * d + (double)mu * (double)sqrtf(fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, eps2))));
+        }
     }
     __shared__ double sh[8];
     __shared__ bool last;
@@ -72,19 +77,23 @@ __global__ void __launch_bounds__(256) tv_trial_kernel(float *__restrict__ buf0,
     const float *f = s->cur ? buf1 : buf0;
     float *t = s->cur ? buf0 : buf1;
     const float tau = s->tau;
-    const long long n = (long long)nx * ny * nz;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((long long)nx * ny));
-        float gx, gy, gz, inv, a, b, c, ninv;
-        tv_diffs(f, x, y, z, nx, ny, nz, eps2, gx, gy, gz, inv);
-        // (D^T p)[i] = sum_a ( p_a[i - e_a] - p_a[i] ),  p = Df / sqrt(|Df|^2 + eps^2)
-        float div = -(gx + gy + gz) * inv;
-        if (x > 0) { tv_diffs(f, x - 1, y, z, nx, ny, nz, eps2, a, b, c, ninv); div = fmaf(a, ninv, div); }
-        if (y > 0) { tv_diffs(f, x, y - 1, z, nx, ny, nz, eps2, a, b, c, ninv); div = fmaf(b, ninv, div); }
-        if (z > 0) { tv_diffs(f, x, y, z - 1, nx, ny, nz, eps2, a, b, c, ninv); div = fmaf(c, ninv, div); }
-        const float fi = __ldg(f + i);
-        const float grad = fmaf(mu, div, 2.f * (fi - __ldg(u + i)));
-        t[i] = fmaf(-tau, grad, fi);
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, ytiles = (ny + 7) >> 3;
+    for (int job = blockIdx.x; job < ytiles * nz; job += gridDim.x) {
+        const int z = job / ytiles, y = (job - z * ytiles) * 8 + ty;
+        if (y >= ny) continue;
+        const size_t row = ((size_t)z * ny + y) * nx;
+        for (int x = tx; x < nx; x += 32) {
+            float gx, gy, gz, inv, a, b, c, ninv;
+            tv_diffs(f, x, y, z, nx, ny, nz, eps2, gx, gy, gz, inv);
+            // (D^T p)[i] = sum_a ( p_a[i - e_a] - p_a[i] ),  p = Df / sqrt(|Df|^2 + eps^2)
+            float div = -(gx + gy + gz) * inv;
+            if (x > 0) { tv_diffs(f, x - 1, y, z, nx, ny, nz, eps2, a, b, c, ninv); div = fmaf(a, ninv, div); }
+            if (y > 0) { tv_diffs(f, x, y - 1, z, nx, ny, nz, eps2, a, b, c, ninv); div = fmaf(b, ninv, div); }
+            if (z > 0) { tv_diffs(f, x, y, z - 1, nx, ny, nz, eps2, a, b, c, ninv); div = fmaf(c, ninv, div); }
+            const float fi = __ldg(f + row + x);
+            const float grad = fmaf(mu, div, 2.f * (fi - __ldg(u + row + x)));
+            t[row + x] = fmaf(-tau, grad, fi);
+        }
     }
 }
 
@@ -122,6 +131,12 @@ static inline int tv_blocks(long long n) {
     if (b > kReduceBlocks) b = kReduceBlocks;
     return (int)(b < 1 ? 1 : b);
 }
+// trial / energy kernels: one block job = 8 rows of one plane (32 x 8 threads, x strides over the row)
+static inline int tv_jobs(int ny, int nz) {
+    long long b = (long long)((ny + 7) >> 3) * nz;
+    if (b > kReduceBlocks) b = kReduceBlocks;
+    return (int)(b < 1 ? 1 : b);
+}
 
 }  // namespace cbct
 
@@ -144,17 +159,17 @@ extern "C" int tv_rof(const float *d_u, float *d_f, void *d_work, float mu_tv, f
     float *buf1 = reinterpret_cast<float *>(w);
     TvState *s = reinterpret_cast<TvState *>(w + align_up(sizeof(float) * (size_t)n, 256));
     double *partials = reinterpret_cast<double *>(w + align_up(sizeof(float) * (size_t)n, 256) + 256);
-    const int blocks = tv_blocks(n);
+    const int blocks = tv_blocks(n), jobs = tv_jobs(ny, nz);
     const float eps2 = eps * eps;
     CBCT_CUDA_TRY(cudaMemcpyAsync(d_f, d_u, sizeof(float) * (size_t)n, cudaMemcpyDeviceToDevice, st));      // descent starts from f = u
     tv_init_kernel<<<1, 1, 0, st>>>(s);
     CBCT_LAUNCH_CHECK();
-    tv_energy_kernel<<<blocks, 256, 0, st>>>(d_f, buf1, d_u, s, 0, mu_tv, eps2, nx, ny, nz, partials);
+    tv_energy_kernel<<<jobs, 256, 0, st>>>(d_f, buf1, d_u, s, 0, mu_tv, eps2, nx, ny, nz, partials);
     CBCT_LAUNCH_CHECK();
     for (int it = 0; it < max_iter; ++it) {
-        tv_trial_kernel<<<blocks, 256, 0, st>>>(d_f, buf1, d_u, s, mu_tv, eps2, nx, ny, nz);
+        tv_trial_kernel<<<jobs, 256, 0, st>>>(d_f, buf1, d_u, s, mu_tv, eps2, nx, ny, nz);
         CBCT_LAUNCH_CHECK();
-        tv_energy_kernel<<<blocks, 256, 0, st>>>(d_f, buf1, d_u, s, 1, mu_tv, eps2, nx, ny, nz, partials);
+        tv_energy_kernel<<<jobs, 256, 0, st>>>(d_f, buf1, d_u, s, 1, mu_tv, eps2, nx, ny, nz, partials);
         CBCT_LAUNCH_CHECK();
         tv_decide_kernel<<<1, 1, 0, st>>>(s, rel_tol);
         CBCT_LAUNCH_CHECK();
