@@ -322,16 +322,18 @@ __global__ void __launch_bounds__(256) backproject_outlier_kernel(DevGeom g, con
     const float t = __uint_as_float(__ldg(ref));
     if (!(t > 0.f && t <= 3.0e38f)) return;
     const float scale = two_qb / t;
-    const long long per_view = (long long)g.nv * g.nu, n = per_view * n_views;
+    // ray counts fit 31 bits (cbct_geometry_create rejects larger detectors): 32-bit index arithmetic, one division per ray
+    const unsigned per_view = (unsigned)g.nv * (unsigned)g.nu, n = per_view * (unsigned)n_views;
     const int lane = threadIdx.x & 31;
-    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long base = warp0 * 32; base < n; base += n_warps * 32) {
-        const long long i = base + lane;
+    const unsigned warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    for (unsigned base = warp0 * 32; base < n; base += n_warps * 32) {
+        const unsigned i = base + lane;
         float gs = 0.f;
         int view = 0, pix = 0;
         if (i < n) {
-            view = g.view_order[view0 + (int)(i / per_view)];
-            pix = (int)(i % per_view);
+            const unsigned vpos = i / per_view;
+            view = g.view_order[view0 + (int)vpos];
+            pix = (int)(i - vpos * per_view);
             gs = __ldg(proj + (size_t)view * per_view + pix) * scale;
         }
         unsigned todo = __ballot_sync(0xffffffffu, i < n && !(fabsf(gs) <= two_qb) && fabsf(gs) <= 3.0e38f);
