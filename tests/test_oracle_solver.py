@@ -109,6 +109,37 @@ def test_collapse_identity_is_a_second_route(mu):
     assert np.max(np.abs(osv.tf_apply(f, mu) - route2)) < 1e-13
 
 
+def _filt(g, axis, l):
+    """h_l along one axis with edge-replicate extension, written out tap by tap (alpha[x] = sum_a h_l[a] g[x - a])"""
+    n = g.shape[axis]
+    pad = [(0, 0)] * g.ndim
+    pad[axis] = (1, 1)
+    e = np.pad(g, pad, mode="edge")
+    sl = lambda k: tuple(slice(k, k + n) if ax == axis else slice(None) for ax in range(g.ndim))
+    return osv.H[l][0] * e[sl(2)] + osv.H[l][1] * e[sl(1)] + osv.H[l][2] * e[sl(0)]        # taps a = -1, 0, +1
+
+
+def test_high_band_energy_from_separable_difference_terms():
+    """The route tf_fused_march_kernel takes: per axis sum_l (h_l * g)^2 = h0 * g^2, hence
+        ||alpha_h||^2 = Wz[ Wy[X_1^2 + X_2^2] + Y_01^2 + Y_02^2 ] + alpha_001^2 + alpha_002^2
+    with X_l = h_l *x f, Y_0m = h_m *y X_0, alpha_00n = h_n *z Y_00 -- a sum of non-negative terms made of difference
+    filters.  Checked against the 26 high bands of the oracle's plain decomposition, faces and 1-thick axes included."""
+    rng = np.random.default_rng(11)
+    for shape in ((6, 7, 8), (1, 5, 9), (4, 1, 3), (2, 2, 1)):
+        f = rng.standard_normal(shape) + 50.0                       # a large offset: the terms below never see it
+        a = osv.tf_decompose(f)
+        X = [_filt(f, 2, l) for l in range(3)]                      # axes: volumes are f[z][y][x], l runs on x
+        assert np.max(np.abs(sum(x * x for x in X) - _filt(f * f, 2, 0))) < 1e-9
+        Y0 = [_filt(X[0], 1, m) for m in range(3)]
+        A00 = [_filt(Y0[0], 0, n) for n in range(3)]
+        t = _filt(X[1] ** 2 + X[2] ** 2, 1, 0) + Y0[1] ** 2 + Y0[2] ** 2
+        energy = _filt(t, 0, 0) + A00[1] ** 2 + A00[2] ** 2
+        assert np.max(np.abs(A00[0] - a[0])) < 1e-12 and np.max(np.abs(A00[2] - a[18])) < 1e-12      # band i = l + 3m + 9n
+        ref = np.sum(a[1:] ** 2, axis=0)
+        assert np.max(np.abs(energy - ref)) <= 1e-12 * max(np.max(ref), 1.0), shape
+        assert np.all(energy >= 0.0)
+
+
 def test_tf_apply_limits():
     rng = np.random.default_rng(10)
     f = rng.standard_normal((4, 5, 6))
