@@ -67,6 +67,9 @@ def shim_as_cuda():
         patch(cb, "_stream", lambda stream=None: 0)
         real_microbench = cb.microbench                            # default loop length (2000) would take hours on the host
         patch(cb, "microbench", lambda stream=None, iters=0: real_microbench(stream, iters if iters > 0 else 1))
+        from paper_1008_2042_b200 import replicas
+        real_init = replicas.init                                  # N > 1 dry runs rendezvous over gloo
+        patch(replicas, "init", lambda backend="nccl", device=None: real_init("gloo", None))
         patch(torch.cuda, "is_available", lambda: True)
         patch(torch.cuda, "set_device", lambda *a, **k: None)
         patch(torch.cuda, "synchronize", lambda *a, **k: None)
