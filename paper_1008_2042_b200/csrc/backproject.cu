@@ -355,13 +355,14 @@ int build_bp_tables(cbct_geometry *G) {
     return CBCT_OK;
 }
 
-int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
+int launch_backproject(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st, double *d_norm, bool *fused) {
     const DevGeom &g = G->dg;
     ProfScope prof(PROF_BACK, st);
     CBCT_TRY(device_error_pending(G));
     // the implementation was fixed at cbct_geometry_create (G->bp_impl): scatter (backproject_tma.cu) where the geometry
     // supports it, else the cell-driven kernel below; gather = the per-voxel cross-check
-    if (G->bp_impl == BP_SCATTER) return launch_backproject_tma(G, d_proj, d_vol, st);
+    if (fused) *fused = d_norm && G->bp_impl == BP_SCATTER;
+    if (G->bp_impl == BP_SCATTER) return launch_backproject_tma(G, d_proj, d_vol, st, d_norm);
     if (G->bp_impl == BP_GATHER) {
         dim3 block(32, 4), grid(cdiv(g.nx, 32), cdiv(g.ny, 4), g.nz);
         backproject_gather_kernel<<<grid, block, 0, st>>>(g, d_proj, d_vol);

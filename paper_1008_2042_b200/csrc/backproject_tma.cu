@@ -387,13 +387,14 @@ __global__ void __launch_bounds__(256) backproject_outlier_kernel(DevGeom g, con
 __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y,
                                                                    float *__restrict__ vol, int nx, int ny, int pf, int ps, int pz,
                                                                    const unsigned *__restrict__ absmax_bits, float step_over_two_qb,
-                                                                   int accumulate, long long sat_limit, DevErr err) {
+                                                                   int accumulate, long long sat_limit, DevErr err, NormOut norm) {
     __shared__ int tile[32][33];
     const size_t base = (size_t)blockIdx.z * nx * ny;
     const size_t base_x = ((size_t)(blockIdx.z + pz) * (ny + ps) + ps) * (nx + pf) + pf;     // acc_x[z+pz][ps][pf]
     const size_t base_y = ((size_t)(blockIdx.z + pz) * (nx + ps) + ps) * (ny + pf) + pf;     // acc_y[z+pz][ps][pf]
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const float k = __uint_as_float(__ldg(absmax_bits)) * step_over_two_qb;         // the fixed-point reference of the caller
+    double sq = 0.0;
     for (int j = threadIdx.y; j < 32; j += 8) {
         const int y = y0 + threadIdx.x, x = x0 + j;
         if (x < nx && y < ny) tile[j][threadIdx.x] = __ldg(acc_y + base_y + (size_t)x * (ny + pf) + y);
@@ -411,9 +412,19 @@ __global__ void __launch_bounds__(256) backproject_finalize_kernel(const int *__
                 atomicOr(err.dev, DEV_ERR_FIXED_POINT);
                 *reinterpret_cast<volatile int *>(err.host) = DEV_ERR_FIXED_POINT;
             }
-            const float v = (float)wide * k;
-            vol[o] = accumulate ? vol[o] + v : v;
+            const float v = (float)wide * k, out = accumulate ? vol[o] + v : v;
+            vol[o] = out;
+            sq = fma((double)out, (double)out, sq);
         }
+    }
+    if (norm.out) {                                        // ||s||^2 of the finished volume (CGLS step 5), fixed summation order
+        __shared__ double sh[8];
+        __shared__ bool last;
+        double tot;
+        const unsigned bid = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+        if (ordered_total_at(sq, norm.partials, norm.counter, sh, &last, tot, threadIdx.y * 32 + threadIdx.x, 256, bid,
+                             gridDim.x * gridDim.y * gridDim.z))
+            *norm.out = tot;
     }
 }
 
@@ -471,6 +482,8 @@ void free_backproject_tma(cbct_geometry *G) {
     cudaFree(G->d_bt_acc);
     cudaFree(G->d_bt_absmax);
     cudaFree(G->d_bt_sumsq); cudaFree(G->d_bt_partials); cudaFree(G->d_bt_counter);
+    cudaFree(G->d_bt_norm_partials); cudaFree(G->d_bt_norm_counter);
+    G->d_bt_norm_partials = nullptr; G->d_bt_norm_counter = nullptr;
     G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr; G->d_bt_sumsq = G->d_bt_partials = nullptr; G->d_bt_counter = nullptr; G->bt_ok = 0;
 }
 
@@ -479,6 +492,7 @@ void plan_backproject_tma(cbct_geometry *G) {
     const cbct_geometry_desc &d = G->desc;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
     G->d_bt_sumsq = G->d_bt_partials = nullptr; G->d_bt_counter = nullptr;
+    G->d_bt_norm_partials = nullptr; G->d_bt_norm_counter = nullptr;
     if (!G->fw_tma_ok) return;
     // lane layout G->bt_lm (see the kernel; chosen by cbct_geometry_create): 0 = the skewed 8x4 layout, whose box is the
     // forward kernel's with the row count rounded up to a multiple of 4 (plane pitch = 0 mod 32); 1 = 16x2, forward's box
@@ -495,7 +509,10 @@ void plan_backproject_tma(cbct_geometry *G) {
     if (cudaMalloc(&G->d_bt_acc, sizeof(int) * G->bt_acc_elems) != cudaSuccess ||
         cudaMalloc(&G->d_bt_absmax, 2 * sizeof(unsigned)) != cudaSuccess || cudaMalloc(&G->d_bt_sumsq, sizeof(double)) != cudaSuccess ||
         cudaMalloc(&G->d_bt_partials, sizeof(double) * kReduceBlocks) != cudaSuccess ||
-        cudaMalloc(&G->d_bt_counter, sizeof(unsigned)) != cudaSuccess || cudaMemset(G->d_bt_counter, 0, sizeof(unsigned)) != cudaSuccess) {
+        cudaMalloc(&G->d_bt_counter, sizeof(unsigned)) != cudaSuccess || cudaMemset(G->d_bt_counter, 0, sizeof(unsigned)) != cudaSuccess ||
+        cudaMalloc(&G->d_bt_norm_partials, sizeof(double) * (size_t)cdiv(d.nx, 32) * cdiv(d.ny, 32) * d.nz) != cudaSuccess ||
+        cudaMalloc(&G->d_bt_norm_counter, sizeof(unsigned int)) != cudaSuccess ||
+        cudaMemset(G->d_bt_norm_counter, 0, sizeof(unsigned int)) != cudaSuccess) {
         (void)cudaGetLastError();
         free_backproject_tma(G);
         return;
@@ -524,7 +541,7 @@ void plan_backproject_tma(cbct_geometry *G) {
     G->bt_ok = 1;
 }
 
-int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st) {
+int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d_vol, cudaStream_t st, double *d_norm) {
     if (!G->bt_ok) return CBCT_E_UNSUPPORTED;
     const DevGeom &g = G->dg;
     CUtensorMap mx, my;
@@ -553,7 +570,8 @@ int launch_backproject_tma(const cbct_geometry *G, const float *d_proj, float *d
         dim3 fb(32, 8), fg(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
         backproject_finalize_kernel<<<fg, fb, 0, st>>>(G->d_bt_acc, G->d_bt_acc + G->bt_acc_y_off, d_vol, g.nx, g.ny, G->bt_b, G->bt_bs,
                                                        G->bt_bz, G->d_bt_absmax + 1,
-                                                       (float)(G->step / std::ldexp(1.0, qb)), v0 > 0 ? 1 : 0, 1LL << 30, G->err);
+                                                       (float)(G->step / std::ldexp(1.0, qb)), v0 > 0 ? 1 : 0, 1LL << 30, G->err,
+                                                       NormOut{v0 + nv_ >= g.n_views ? d_norm : nullptr, G->d_bt_norm_partials, G->d_bt_norm_counter});
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;

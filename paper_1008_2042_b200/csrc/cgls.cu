@@ -2,7 +2,8 @@
 // The paper uses CUBLAS for the vector-vector operations; here they are fused
 // kernels whose scalars (gamma, ||q||^2, alpha, beta) never leave the device, so a step is a fixed
 // launch sequence with no host synchronisation.  Reductions accumulate in fp64 and are summed in a
-// fixed order (deterministic).
+// fixed order (deterministic).  ||q||^2 and ||s||^2 are delivered by the projector launches themselves where the
+// TMA kernels serve the handle (epilogue of P, conversion pass of P^T: SURVEY.md §8(d) "fused minimum").
 #include <new>
 
 #include "common.cuh"
@@ -158,8 +159,9 @@ extern "C" int cbct_cgls_init(cbct_cgls *cg, const float *d_g, const float *d_x,
     CBCT_TRY(launch_forward(G, d_x, cg->d_q, st));                                   // q = P x0
     residual_kernel<<<ew_blocks(G->n_rays), 256, 0, st>>>(d_r, d_g, cg->d_q, G->n_rays);   // r = g - P x0
     CBCT_LAUNCH_CHECK();
-    CBCT_TRY(launch_backproject(G, d_r, d_p, st));                                   // p = s = P^T r
-    CBCT_TRY(launch_sumsq(d_p, G->n_vox, cg->d_scal + S_GAMMA_NEW, cg->d_partials, cg->d_counter, st));
+    bool fused = false;
+    CBCT_TRY(launch_backproject(G, d_r, d_p, st, cg->d_scal + S_GAMMA_NEW, &fused));  // p = s = P^T r, ||s||^2 from its conversion pass
+    if (!fused) CBCT_TRY(launch_sumsq(d_p, G->n_vox, cg->d_scal + S_GAMMA_NEW, cg->d_partials, cg->d_counter, st));
     cgls_set_gamma_kernel<<<1, 1, 0, st>>>(cg->d_scal);                              // gamma = ||s||^2
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
@@ -169,16 +171,17 @@ extern "C" int cbct_cgls_step(cbct_cgls *cg, float *d_x, float *d_r, float *d_p,
     if (!cg || !d_x || !d_r || !d_p) return CBCT_E_INVALID;
     cudaStream_t st = as_stream(stream);
     const cbct_geometry *G = cg->geom;
-    CBCT_TRY(launch_forward(G, d_p, cg->d_q, st));                                                   // 1. q = P p
-    CBCT_TRY(launch_sumsq(cg->d_q, G->n_rays, cg->d_scal + S_QQ, cg->d_partials, cg->d_counter, st));
+    bool fused = false;
+    CBCT_TRY(launch_forward(G, d_p, cg->d_q, st, cg->d_scal + S_QQ, &fused));                        // 1. q = P p, ||q||^2 from its epilogue
+    if (!fused) CBCT_TRY(launch_sumsq(cg->d_q, G->n_rays, cg->d_scal + S_QQ, cg->d_partials, cg->d_counter, st));
     cgls_alpha_kernel<<<1, 1, 0, st>>>(cg->d_scal, cg->d_flag);                                      // 2. alpha
     CBCT_LAUNCH_CHECK();
     axpy_dev_kernel<<<ew_blocks(G->n_vox), 256, 0, st>>>(d_x, d_p, G->n_vox, cg->d_scal, 1.f);       // 3. x += alpha p
     CBCT_LAUNCH_CHECK();
     axpy_dev_kernel<<<ew_blocks(G->n_rays), 256, 0, st>>>(d_r, cg->d_q, G->n_rays, cg->d_scal, -1.f); //    r -= alpha q
     CBCT_LAUNCH_CHECK();
-    CBCT_TRY(launch_backproject(G, d_r, cg->d_s, st));                                               // 4. s = P^T r
-    CBCT_TRY(launch_sumsq(cg->d_s, G->n_vox, cg->d_scal + S_GAMMA_NEW, cg->d_partials, cg->d_counter, st));  // 5.
+    CBCT_TRY(launch_backproject(G, d_r, cg->d_s, st, cg->d_scal + S_GAMMA_NEW, &fused));             // 4. s = P^T r, 5. ||s||^2
+    if (!fused) CBCT_TRY(launch_sumsq(cg->d_s, G->n_vox, cg->d_scal + S_GAMMA_NEW, cg->d_partials, cg->d_counter, st));
     cgls_beta_kernel<<<1, 1, 0, st>>>(cg->d_scal, cg->d_flag);                                       // 6. beta
     CBCT_LAUNCH_CHECK();
     p_update_kernel<<<ew_blocks(G->n_vox), 256, 0, st>>>(d_p, cg->d_s, G->n_vox, cg->d_scal, cg->d_flag);    // 7.

@@ -93,33 +93,40 @@ __device__ __forceinline__ void ray_setup(const DevGeom &g, int view, int iv, in
 // done by the whole block (thread t takes partials t, t + 256, ..., then the same warp / block tree), not by one thread
 // walking gridDim.x dependent loads from L2 -- with 1184 blocks that walk was most of the kernel's time in round 1.
 // `sh` = 8 doubles and `last` = one bool of shared memory, both declared by the calling kernel.
-__device__ __forceinline__ bool ordered_total(double acc, double *partials, unsigned int *counter, double *sh, bool *last, double &total) {
+__device__ __forceinline__ bool ordered_total_at(double acc, double *partials, unsigned int *counter, double *sh, bool *last, double &total,
+                                                 unsigned tid, unsigned n_threads, unsigned bid, unsigned n_blocks) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+    if ((tid & 31) == 0) sh[tid >> 5] = acc;
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
         double s = 0.0;
         for (int w = 0; w < 8; ++w) s += sh[w];
-        partials[blockIdx.x] = s;
+        partials[bid] = s;
         __threadfence();
-        *last = (atomicAdd(counter, 1u) == gridDim.x - 1);
+        *last = (atomicAdd(counter, 1u) == n_blocks - 1);
     }
     __syncthreads();
     if (!*last) return false;                                    // block-uniform
     __threadfence();
     double s = 0.0;
-    for (unsigned b = threadIdx.x; b < gridDim.x; b += blockDim.x) s += ((volatile double *)partials)[b];
+    for (unsigned b = tid; b < n_blocks; b += n_threads) s += ((volatile double *)partials)[b];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;       // thread 0 read sh before the barrier above: no hazard
+    if ((tid & 31) == 0) sh[tid >> 5] = s;                        // thread 0 read sh before the barrier above: no hazard
     __syncthreads();
-    if (threadIdx.x != 0) return false;
+    if (tid != 0) return false;
     total = 0.0;
     for (int w = 0; w < 8; ++w) total += sh[w];
     *counter = 0u;
     return true;
 }
+__device__ __forceinline__ bool ordered_total(double acc, double *partials, unsigned int *counter, double *sh, bool *last, double &total) {
+    return ordered_total_at(acc, partials, counter, sh, last, total, threadIdx.x, blockDim.x, blockIdx.x, gridDim.x);
+}
+// where a kernel leaves the squared norm of its OUTPUT (SURVEY.md §8(d) "fused minimum": ||q||^2 in the epilogue of P, ||s||^2
+// in the conversion pass of P^T); out == nullptr: not wanted
+struct NormOut { double *out; double *partials; unsigned int *counter; };
 
 // ---- P^T (cell-driven) tables, built in fp64 at geometry create, stored fp32 ------------------------
 // With r = t / L(u,v) (t = distance from the source) a ray is  X = Kx + Ax r,  Y = Ky + Ay r,  Z = Kz + vz r,
@@ -176,6 +183,8 @@ struct cbct_geometry {
     int fw_tma_ok, fw_b, fw_bs, fw_bz;      // box: fw_b columns (= row pitch) x fw_bs rows x fw_bz planes
     float fw_margin;
     float *d_fw_volT;
+    double *d_fw_norm_partials;             // ||q||^2 block partials of forward_tma_kernel (one per CTA) + its counter
+    unsigned int *d_fw_norm_counter;
     alignas(64) unsigned char fw_map_y[128];
     // P^T scatter path (backproject_tma.cu): int32 accumulator volumes (x-fastest, then y-fastest), max|g|, fixed-point plan
     int bt_b, bt_bs, bt_bz;                 // accumulator box (row pitch bt_b, bt_bs rows, bt_bz planes)
@@ -186,6 +195,8 @@ struct cbct_geometry {
     unsigned *d_bt_absmax;                  // [0] bits of max|g|, [1] bits of the fixed-point reference T = min(max|g|, 8 rms(g))
     double *d_bt_sumsq, *d_bt_partials;     // ||g||^2 (deterministic two-level reduction) and its scratch
     unsigned *d_bt_counter;
+    double *d_bt_norm_partials;             // ||s||^2 block partials of the conversion pass (one per block) + its counter
+    unsigned int *d_bt_norm_counter;
     alignas(64) unsigned char bt_map_x[128];
     alignas(64) unsigned char bt_map_y[128];
     // Siddon pair (siddon.cu), allocated by cbct_siddon_prepare: y-fastest volume copy, two int32 accumulator volumes, max|g|
@@ -216,14 +227,16 @@ static inline int device_error_pending(const cbct_geometry *G) {
     return (G->h_err && *reinterpret_cast<volatile int *>(G->h_err)) ? CBCT_E_DEVICE : CBCT_OK;
 }
 // kernels' host launchers used across translation units
-int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
-int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
+// d_norm != nullptr: the caller wants ||output||^2 (fp64, device) from the same launch; *fused says whether the kernel that
+// served the handle delivered it (the TMA kernels do: SURVEY.md §8(d) "fused minimum"), else the caller reduces the output itself
+int launch_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st, double *d_norm = nullptr, bool *fused = nullptr);
+int launch_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st, double *d_norm = nullptr, bool *fused = nullptr);
 void plan_forward_tma(cbct_geometry *g);     // decides whether/how the TMA forward kernel runs for this geometry
-int launch_forward_tma(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st);
+int launch_forward_tma(const cbct_geometry *g, const float *d_vol, float *d_proj, cudaStream_t st, double *d_norm = nullptr);
 void plan_backproject_tma(cbct_geometry *g); // after plan_forward_tma: same boxes, int32 accumulators
 void free_backproject_tma(cbct_geometry *g);
 bool bt_fixed_point_plan(const cbct_geometry_desc &d, double R, double step, int *qb, int *views_per_group, double *w_view);
-int launch_backproject_tma(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st);
+int launch_backproject_tma(const cbct_geometry *g, const float *d_proj, float *d_vol, cudaStream_t st, double *d_norm = nullptr);
 void free_siddon(cbct_geometry *g);
 bool siddon_fixed_point_plan(const cbct_geometry_desc &d, double R, int *qb, int *views_per_group, double *w_view);
 // kernels launched from more than one translation unit
@@ -231,7 +244,7 @@ __global__ void transpose_vol_kernel(const float *__restrict__ v, float *__restr
 __global__ void absmax_kernel(const float *__restrict__ g, long long n, unsigned *out);                        // backproject_tma.cu
 __global__ void backproject_finalize_kernel(const int *__restrict__ acc_x, const int *__restrict__ acc_y, float *__restrict__ vol,
                                             int nx, int ny, int pf, int ps, int pz, const unsigned *__restrict__ absmax_bits,
-                                            float step_over_two_qb, int accumulate, long long sat_limit, DevErr err);  // backproject_tma.cu
+                                            float step_over_two_qb, int accumulate, long long sat_limit, DevErr err, NormOut norm);  // backproject_tma.cu
 int build_bp_tables(cbct_geometry *g);      // allocates + fills g->bp and g->d_bp_partial
 void free_bp_tables(cbct_geometry *g);
 int launch_sumsq(const float *d_v, int64_t n, double *d_out, double *d_partials, unsigned int *d_counter,

@@ -232,13 +232,14 @@ bool forward_tiled_fits(const cbct_geometry *G, float *margin_out) {
     return exy * exy * ez <= 1.5 * FW_CAP && margin < 4.0;
 }
 
-int launch_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st) {
+int launch_forward(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st, double *d_norm, bool *fused) {
     const DevGeom &g = G->dg;
     ProfScope prof(PROF_FORWARD, st);
     dim3 block(FW_TU, FW_TV), grid(cdiv(g.nu, FW_TU), cdiv(g.nv, FW_TV), g.n_views);
     CBCT_TRY(device_error_pending(G));
     // the implementation was fixed at cbct_geometry_create (G->fw_impl): a failure here is returned, never re-routed
-    if (G->fw_impl == FW_TMA) return launch_forward_tma(G, d_vol, d_proj, st);
+    if (fused) *fused = d_norm && G->fw_impl == FW_TMA;
+    if (G->fw_impl == FW_TMA) return launch_forward_tma(G, d_vol, d_proj, st, d_norm);
     float margin = 0.f;
     if (G->fw_impl == FW_TILED) {
         if (!forward_tiled_fits(G, &margin)) return CBCT_E_UNSUPPORTED;

@@ -33,7 +33,7 @@ template <int BF, int BS, bool PK>
 __global__ void __launch_bounds__(FT_THREADS, 3) forward_tma_kernel(DevGeom g, const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_y,
                                                                  const float *__restrict__ vol, float *__restrict__ proj,
-                                                                 float margin, int bfs, int bss, int bzz, DevErr err) {
+                                                                 float margin, int bfs, int bss, int bzz, DevErr err, NormOut norm) {
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2];
     __shared__ RayL corner[4];
@@ -270,7 +270,17 @@ __global__ void __launch_bounds__(FT_THREADS, 3) forward_tma_kernel(DevGeom g, c
             k0 = kn; stage ^= 1;
         }
     }
-    if (valid) proj[((size_t)view * g.nv + iv) * g.nu + iu] = total * stepf;
+    const float qv = total * stepf;
+    if (valid) proj[((size_t)view * g.nv + iv) * g.nu + iu] = qv;
+    if (norm.out) {                                        // ||q||^2 of this launch (CGLS step 2), fixed summation order
+        __shared__ double sh[8];
+        __shared__ bool last;
+        double tot;
+        const unsigned bid = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+        if (ordered_total_at(valid ? (double)qv * qv : 0.0, norm.partials, norm.counter, sh, &last, tot, tid, FT_THREADS, bid,
+                             gridDim.x * gridDim.y * gridDim.z))
+            *norm.out = tot;
+    }
 }
 
 // volT[z][x][y] = vol[z][y][x]
@@ -290,7 +300,7 @@ __global__ void __launch_bounds__(256) transpose_vol_kernel(const float *__restr
 }
 
 
-typedef void (*TmaKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, float *, float, int, int, int, DevErr);
+typedef void (*TmaKernel)(DevGeom, const CUtensorMap, const CUtensorMap, const float *, float *, float, int, int, int, DevErr, NormOut);
 static TmaKernel tma_kernel_ptr(int bf, int bs, bool pk) {
 #define CBCT_FK(F, S) if (bf == F && bs == S) return pk ? forward_tma_kernel<F, S, true> : forward_tma_kernel<F, S, false>;
     CBCT_FK(24, 22) CBCT_FK(40, 30) CBCT_FK(40, 38) CBCT_FK(56, 46) CBCT_FK(56, 54)
@@ -332,6 +342,13 @@ void plan_forward_tma(cbct_geometry *G) {
     G->fw_b = bf; G->fw_bs = bs; G->fw_bz = bz; G->fw_margin = (float)margin;
     if (cudaMalloc(&G->d_fw_volT, sizeof(float) * G->n_vox) != cudaSuccess) { (void)cudaGetLastError(); G->d_fw_volT = nullptr; return; }
     G->workspace_bytes += sizeof(float) * G->n_vox;
+    {   // ||q||^2 in the kernel's epilogue: one fp64 partial per CTA
+        const size_t n_cta = (size_t)cdiv(d.nu, FT_TU) * cdiv(d.nv, FT_TV) * d.n_views;
+        if (cudaMalloc(&G->d_fw_norm_partials, sizeof(double) * n_cta) != cudaSuccess ||
+            cudaMalloc(&G->d_fw_norm_counter, sizeof(unsigned int)) != cudaSuccess ||
+            cudaMemset(G->d_fw_norm_counter, 0, sizeof(unsigned int)) != cudaSuccess) { (void)cudaGetLastError(); return; }
+        G->workspace_bytes += sizeof(double) * n_cta;
+    }
     static_assert(sizeof(CUtensorMap) <= sizeof(G->fw_map_y), "tensor map storage");
     CUtensorMap m;
     if (!make_map(&m, G->d_fw_volT, d.ny, d.nx, d.nz, bf, bs, bz)) return;
@@ -347,7 +364,7 @@ void plan_forward_tma(cbct_geometry *G) {
     G->fw_tma_ok = 1;
 }
 
-int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st) {
+int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj, cudaStream_t st, double *d_norm) {
     if (!G->fw_tma_ok) return CBCT_E_UNSUPPORTED;
     if (reinterpret_cast<uintptr_t>(d_vol) & 15) return CBCT_E_INVALID;        // include/cbct.h: device pointers are 16-byte aligned
     const DevGeom &g = G->dg;
@@ -363,7 +380,8 @@ int launch_forward_tma(const cbct_geometry *G, const float *d_vol, float *d_proj
     dim3 grid(cdiv(g.nu, FT_TU), cdiv(g.nv, FT_TV), g.n_views);
     TmaKernel kern = tma_kernel_ptr(G->fw_b, G->fw_bs, G->fw_packed != 0);
     if (!kern) return CBCT_E_UNSUPPORTED;
-    kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz, G->err);
+    kern<<<grid, FT_THREADS, smem, st>>>(g, mx, my, d_vol, d_proj, G->fw_margin, G->fw_b, G->fw_bs, G->fw_bz, G->err,
+                                        NormOut{d_norm, G->d_fw_norm_partials, G->d_fw_norm_counter});
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

@@ -272,7 +272,7 @@ static int create_with_options(const cbct_geometry_desc *desc, Options opt, cbct
     G->n_vox = (int64_t)desc->nx * desc->ny * desc->nz;
     G->n_rays = (int64_t)desc->nu * desc->nv * desc->n_views;
     G->d_view_order = nullptr;
-    G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr; G->d_fw_volT = nullptr; G->fw_tma_ok = 0;
+    G->d_view_cs = nullptr; G->d_ws_vol = nullptr; G->d_ws_proj = nullptr; G->d_bp_partial = nullptr; G->d_bp_projT = nullptr; G->d_fw_volT = nullptr; G->d_fw_norm_partials = nullptr; G->d_fw_norm_counter = nullptr; G->fw_tma_ok = 0;
     G->err = DevErr{nullptr, nullptr}; G->h_err = nullptr;
     G->bt_ok = 0; G->d_bt_acc = nullptr; G->d_bt_absmax = nullptr;
     G->d_sd_volT = nullptr; G->d_sd_acc = nullptr; G->d_sd_absmax = nullptr; G->sd_qb = 0; G->sd_group = 0;
@@ -418,6 +418,8 @@ extern "C" int cbct_geometry_destroy(cbct_geometry *G) {
     free_bp_tables(G);
     free_backproject_tma(G);
     cudaFree(G->d_fw_volT);
+    cudaFree(G->d_fw_norm_partials);
+    cudaFree(G->d_fw_norm_counter);
     free_siddon(G);
     (void)cudaGetLastError();
     delete G;

@@ -250,7 +250,7 @@ extern "C" int cbct_siddon_backproject(const cbct_geometry *G, const float *d_pr
         // vol (+)= (acc_x + acc_y^T) * max|g| / 2^qb : the finalize pass of backproject_tma.cu with no margins and unit step
         dim3 fb(32, 8), fg(cdiv(g.nx, 32), cdiv(g.ny, 32), g.nz);
         backproject_finalize_kernel<<<fg, fb, 0, st>>>(G->d_sd_acc, G->d_sd_acc + G->n_vox, d_vol, g.nx, g.ny, 0, 0, 0, G->d_sd_absmax,
-                                                       (float)std::ldexp(1.0, -G->sd_qb), v0 > 0 ? 1 : 0, 1LL << 31, G->err);   // rigorous bound: no head-room check
+                                                       (float)std::ldexp(1.0, -G->sd_qb), v0 > 0 ? 1 : 0, 1LL << 31, G->err, NormOut{nullptr, nullptr, nullptr});   // rigorous bound: no head-room check
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;

@@ -245,3 +245,31 @@ def test_microbench_kernels_stay_in_bounds():
         sl.check(sl.lib().cbct_microbench(kind, 1, out, None), f"cbct_microbench({kind})")
         assert out[2] > 0
     assert sl.lib().cbct_microbench(8, 1, out, None) == -1
+
+
+def test_cgls_step_takes_its_norms_from_the_projector_launches():
+    """SURVEY.md §8(d) "fused minimum": on a handle served by the TMA kernels ||q||^2 comes out of the epilogue of P and
+    ||s||^2 out of the conversion pass of P^T -- no separate pass over q or s (the one sumsq_kernel left in a step is the
+    rms of the P^T INPUT for its fixed-point reference).  A handle served by the plain kernels reduces q and s itself.
+    Either way the scalars are the oracle's."""
+    w, _, f0, g = syn.make_inputs(1)
+    several_groups = syn.Geometry(32, 32, 8, 4.0, 4.0, 4.0, 64, 24, 1.6, 1.6, 1000.0, 1500.0, syn.full_circle(12), step_mm=0.5)
+    assert "views/group 2" in sl.Geometry(several_groups).describe()      # ||s||^2 must come from the LAST of six conversion passes
+    for G, n_sumsq, fwd in ((w.geometry, 1, "cbct::forward_tma_kernel"), (several_groups, 1, "cbct::forward_tma_kernel"),
+                            (syn.Geometry(37, 29, 11, 2.0, 3.0, 5.0, 45, 19, 2.3, 3.1, 1000.0, 1500.0, (0.0, 0.4, 2.0, 4.0)), 2, "cbct::forward_")):
+        P, PT = ops(G)
+        gg = syn.uniform_projections(G, 3) if G is not w.geometry else g
+        h = sl.Geometry(G)
+        cg = sl.Cgls(h)
+        d_x, d_r, d_p = sl.dev(np.zeros(h.vol_shape)), sl.Buf(h.proj_shape), sl.Buf(h.vol_shape)
+        cg.init(sl.dev(gg), d_x, d_r, d_p)
+        st = osv.cgls_init(P, PT, np.zeros(G.vol_shape), gg.astype(np.float64))
+        assert abs(cg.scalars()["gamma"] - st["gamma"]) <= 2e-5 * st["gamma"]
+        sl.kernel_log()
+        cg.step(d_x, d_r, d_p)
+        log = sl.kernel_log()
+        assert sum(k == "cbct::sumsq_kernel" for k in log) == n_sumsq and any(k.startswith(fwd) for k in log), log
+        st = osv.cgls_step(P, PT, st)
+        sc = cg.scalars()
+        assert abs(sc["qq"] - st["qq"]) <= 2e-5 * st["qq"] and abs(sc["gamma"] - st["gamma"]) <= 2e-5 * st["gamma"]
+        assert abs(sc["alpha"] - st["alpha"]) <= 2e-5 * abs(st["alpha"]) and abs(sc["beta"] - st["beta"]) <= 5e-5 * abs(st["beta"])

@@ -110,6 +110,29 @@ def test_cgls_ten_steps_divergence_is_reported_not_hidden():
     assert err <= 1e-3
 
 
+def test_cgls_norms_from_the_projector_launches_with_several_accumulation_groups():
+    """||q||^2 comes out of the epilogue of P and ||s||^2 out of the LAST conversion pass of P^T (SURVEY.md §8(d) "fused
+    minimum"); here P^T needs six accumulation groups (views/group 2), and the scalars must still be the oracle's."""
+    G = syn.Geometry(32, 32, 8, 4.0, 4.0, 4.0, 64, 24, 1.6, 1.6, 1000.0, 1500.0, syn.full_circle(12), step_mm=0.5)
+    P, PT = ops(G)
+    g = syn.uniform_projections(G, 3)
+    h = cb.Geometry(G)
+    print(h.describe())
+    cg = cb.Cgls(h)
+    d_x = torch.zeros(h.vol_shape, dtype=torch.float32, device="cuda")
+    d_r = torch.empty(h.proj_shape, dtype=torch.float32, device="cuda")
+    d_p = torch.empty(h.vol_shape, dtype=torch.float32, device="cuda")
+    cg.init(dev(g), d_x, d_r, d_p)
+    st = osv.cgls_init(P, PT, np.zeros(G.vol_shape), g.astype(np.float64))
+    assert abs(cg.scalars()["gamma"] - st["gamma"]) <= 2e-5 * st["gamma"]
+    for _ in range(2):
+        cg.step(d_x, d_r, d_p)
+        st = osv.cgls_step(P, PT, st)
+        sc = cg.scalars()
+        assert abs(sc["qq"] - st["qq"]) <= 5e-5 * st["qq"] and abs(sc["gamma"] - st["gamma"]) <= 5e-5 * st["gamma"]
+    assert rel(host(d_x), st["x"]) <= 1e-4 and h.status() == (True, [])
+
+
 def test_cgls_breakdown_flag():
     G = syn.workload(1).geometry
     h = cb.Geometry(G)
